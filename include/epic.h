@@ -1,0 +1,133 @@
+/* epic.h — C ABI of libepic.so: the EPIC (E-field Parallel Imaging Correlator) hot path on
+ * one NVIDIA B200 (sm_100a).
+ *
+ * Method: Kent et al., arXiv 1904.11422.  Per frequency channel c and time sample t
+ * (one "frame"), per polarisation p (Eq. 5; §3.2):
+ *
+ *   S1 unpack      byte -> E = sext4(byte >> 4) + i sext4(byte & 15)
+ *   S2 cells       nearest cell (cx,cy) = floor(u+0.5), floor(v+0.5); tap cell
+ *                  ((cy+dy) mod N, (cx+dx) mod N)
+ *   S3 gridding    G[y][x] += W_a[dy][dx] * E_a   (collisions sum)
+ *   S4 transform   A[m][l] = sum_{y,x} G[y][x] exp(+2 pi i (x l + y m)/N)          PAPER.md:126, Eq. 5
+ *   S5 products    XX=|A_X|^2, YY=|A_Y|^2, XY=A_X conj(A_Y), YX=A_Y conj(A_X)
+ *   S6 accumulate  sum over the n_t time samples of the call
+ *
+ * N = grid_n * pad (zero-padded plane side, a power of two).  The transform is the
+ * unnormalised inverse DFT in natural order with zenith (l = m = 0) at [0][0]; no fftshift.
+ * All arithmetic is fp32 (the paper's complex64).
+ *
+ * Conventions.  Every function returns EPIC_OK (0) or a negative epic_status; nothing throws
+ * across the ABI.  Argument validation is synchronous.  Device work is enqueued on `stream`
+ * (a cudaStream_t passed as void*; NULL = the legacy default stream) and is asynchronous:
+ * kernel faults surface at the caller's next synchronisation.  epic_image* never allocate,
+ * never synchronise with the host and never copy host memory.  A plan owns device tables and
+ * a scratch buffer; calls on ONE plan must be issued on one stream at a time (the scratch is
+ * per plan).  Pointers marked HOST are read during the call and not retained; pointers marked
+ * DEVICE are owned by the caller (e.g. PyTorch tensors) and must stay valid until the
+ * enqueued work has finished.
+ */
+#ifndef EPIC_H_
+#define EPIC_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define EPIC_API __attribute__((visibility("default")))
+#else
+#define EPIC_API
+#endif
+
+typedef struct epic_plan epic_plan; /* opaque; created/destroyed by the library */
+typedef void* epic_stream;          /* cudaStream_t */
+
+typedef enum epic_status {
+  EPIC_OK = 0,
+  EPIC_ERR_ARG = -1,   /* NULL pointer, bad shape, even kernel_k, N not a power of two in 8..512 */
+  EPIC_ERR_RANGE = -2, /* n_pol not in {1,2}, n_products incompatible with n_pol, n_ant too large */
+  EPIC_ERR_CUDA = -3,  /* a CUDA runtime call failed; see epic_last_cuda_error() */
+  EPIC_ERR_NOMEM = -4  /* host or device allocation failed */
+} epic_status;
+
+/* Which kernel family epic_image uses.  AUTO picks the fastest one that supports the plan. */
+typedef enum epic_path {
+  EPIC_PATH_AUTO = 0,
+  EPIC_PATH_TWOPASS = 1, /* grid+row-FFT kernel -> L2-resident scratch -> column-FFT+products kernel */
+  EPIC_PATH_FUSED = 2    /* one kernel, planes never leave the SM (N <= 128 supports only) */
+} epic_path;
+
+/* S2 + plan set-up ("gridded onto a 2D grid ... spacing < lambda/2"; illumination
+ * kernel "user-defined").  HOST pointers, copied.
+ *   grid_n, pad   aperture cells per side and integer zero-padding factor; N = grid_n*pad must be
+ *                 a power of two with 8 <= N <= 512.
+ *   n_ant         number of antennas, 1..65535.
+ *   ant_uv        float[n_ant][2] = (u, v) in aperture CELL units; u -> x -> l is the fast axis.
+ *                 Cell = floor(double(u) + 0.5); cells outside [0,N) wrap modulo N.
+ *   kernel_taps   NULL -> delta kernel (kernel_k must be 1, tap 1+0i); else
+ *                 float[n_ant][kernel_k][kernel_k][2], complex fp32 indexed [dy+h][dx+h],
+ *                 h = (kernel_k-1)/2, shared by both polarisations.
+ *   kernel_k      odd, 1..15.
+ * On success *out receives the plan (products default: n_pol==2 -> 4, n_pol==1 -> 1). */
+EPIC_API int epic_plan_create(epic_plan** out, int grid_n, int pad, int n_ant, const float* ant_uv,
+                     const float* kernel_taps, int kernel_k);
+
+/* Frees the plan's device tables and scratch.  NULL is a no-op.  Synchronises the device. */
+EPIC_API int epic_plan_destroy(epic_plan* plan);
+
+/* S5 selection: n_products = 1 (XX; n_pol must be 1), 2 (XX,YY) or 4 (XX,YY,XY,YX); the latter
+ * two need n_pol == 2.  Checked against n_pol at epic_image time.  0 restores the default. */
+EPIC_API int epic_plan_set_products(epic_plan* plan, int n_products);
+
+/* Select the kernel family (testing / benchmarking).  EPIC_ERR_RANGE if the plan cannot use it. */
+EPIC_API int epic_plan_set_path(epic_plan* plan, int path);
+
+/* S1..S6 for one gulp (one call = one gulp of n_t samples).
+ *   voltages   DEVICE uint8[n_t][n_chan][n_pol][n_ant] — [Time, Channel, Polarisation, Antenna]
+ *              order, 1 byte = 4+4-bit complex: high nibble real, low nibble
+ *              imaginary, two's complement -8..7.
+ *   out_accum  DEVICE float[n_chan][planes][N][N]; planes = 1 {XX} | 2 {XX,YY} |
+ *              6 {XX,YY,Re XY,Im XY,Re YX,Im YX}.  The call ADDS the sum over its n_t samples
+ *              into out_accum ("accumulated"); the caller zeroes it to start an
+ *              integration.  n_t == 0 or n_chan == 0 is a successful no-op. */
+EPIC_API int epic_image(epic_plan* plan, const void* voltages, int n_t, int n_chan, int n_pol,
+               float* out_accum, epic_stream stream);
+
+/* Same with complex fp32 voltages: DEVICE float[n_t][n_chan][n_pol][n_ant][2] (re, im). */
+EPIC_API int epic_image_cf32(epic_plan* plan, const void* voltages_cf32, int n_t, int n_chan, int n_pol,
+                    float* out_accum, epic_stream stream);
+
+/* Plan queries (host, synchronous). */
+EPIC_API int epic_plan_get_n(const epic_plan* plan);        /* N, or negative status */
+EPIC_API int epic_plan_get_n_planes(const epic_plan* plan, int n_pol); /* planes for current products */
+/* S2 result: cells_host HOST int[n_ant][kernel_k][kernel_k] = y*N + x of every tap. */
+EPIC_API int epic_plan_get_cells(const epic_plan* plan, int* cells_host);
+/* Circular bounding box of the occupied cells: HOST int[4] = {y0, x0, rows, cols}. */
+EPIC_API int epic_plan_get_support(const epic_plan* plan, int* box_host);
+/* Kernel family epic_image will use for this plan and n_pol (an epic_path value). */
+EPIC_API int epic_plan_get_path(const epic_plan* plan, int n_pol);
+/* Number of kernel launches the last epic_image* call on this plan enqueued. */
+EPIC_API int epic_plan_last_launches(const epic_plan* plan);
+
+/* Test hooks for the bit-exact clauses (BASELINE.json north_star).
+ * epic_debug_unpack: S1 alone. bytes_dev DEVICE uint8[n] -> out_dev DEVICE float[n][2].
+ * epic_debug_grid:   S1+S3 for ONE frame through the plan's gather table.  voltages DEVICE as
+ *                    in epic_image (is_cf32 != 0: as in epic_image_cf32) with n_t = n_chan = 1;
+ *                    out_plane_dev DEVICE float[n_pol][N][N][2], overwritten, true
+ *                    (un-relocated) cell positions. */
+EPIC_API int epic_debug_unpack(const void* bytes_dev, long n, float* out_dev, epic_stream stream);
+EPIC_API int epic_debug_grid(epic_plan* plan, const void* voltages, int is_cf32, int n_pol,
+                    float* out_plane_dev, epic_stream stream);
+
+/* FP32 FMA micro-benchmark used for the roofline denominator: runs `iters` dependent-chain
+ * FFMA rounds on every SM and writes elapsed milliseconds and the flop count (HOST outputs).
+ * Synchronous. */
+EPIC_API int epic_fp32_peak_probe(int iters, float* ms_out, double* flops_out);
+
+EPIC_API const char* epic_status_string(int status);
+EPIC_API int epic_last_cuda_error(void); /* cudaError_t of the most recent failing CUDA call, per thread */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EPIC_H_ */

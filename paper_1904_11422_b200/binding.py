@@ -1,0 +1,209 @@
+"""ctypes binding of libepic.so (include/epic.h).  Argument marshalling only: every step of the
+EPIC path (unpack, gridding, transform, products, accumulation) runs in the
+library's CUDA kernels.  PyTorch is used for device memory and streams.  There is no CPU
+fallback: a missing library raises."""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libepic.so")
+
+EPIC_OK = 0
+EPIC_ERR_ARG, EPIC_ERR_RANGE, EPIC_ERR_CUDA, EPIC_ERR_NOMEM = -1, -2, -3, -4
+EPIC_PATH_AUTO, EPIC_PATH_TWOPASS, EPIC_PATH_FUSED = 0, 1, 2
+
+# every symbol include/epic.h declares: name -> (restype, argtypes)
+_vp, _i, _l = ctypes.c_void_p, ctypes.c_int, ctypes.c_long
+SYMBOLS = {
+    "epic_plan_create": (_i, [ctypes.POINTER(_vp), _i, _i, _i, _vp, _vp, _i]),
+    "epic_plan_destroy": (_i, [_vp]),
+    "epic_plan_set_products": (_i, [_vp, _i]),
+    "epic_plan_set_path": (_i, [_vp, _i]),
+    "epic_image": (_i, [_vp, _vp, _i, _i, _i, _vp, _vp]),
+    "epic_image_cf32": (_i, [_vp, _vp, _i, _i, _i, _vp, _vp]),
+    "epic_plan_get_n": (_i, [_vp]),
+    "epic_plan_get_n_planes": (_i, [_vp, _i]),
+    "epic_plan_get_cells": (_i, [_vp, _vp]),
+    "epic_plan_get_support": (_i, [_vp, _vp]),
+    "epic_plan_get_path": (_i, [_vp, _i]),
+    "epic_plan_last_launches": (_i, [_vp]),
+    "epic_debug_unpack": (_i, [_vp, _l, _vp, _vp]),
+    "epic_debug_grid": (_i, [_vp, _vp, _i, _i, _vp, _vp]),
+    "epic_fp32_peak_probe": (_i, [_i, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_double)]),
+    "epic_status_string": (ctypes.c_char_p, [_i]),
+    "epic_last_cuda_error": (_i, []),
+}
+
+_lib = None
+
+
+class EpicError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = lib().epic_status_string(status).decode()
+        if status == EPIC_ERR_CUDA:
+            msg += f" (cudaError {lib().epic_last_cuda_error()})"
+        super().__init__(f"{where}: {msg}")
+
+
+def lib() -> ctypes.CDLL:
+    """The loaded libepic.so.  Raises if it has not been built (python -m paper_1904_11422_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_1904_11422_b200.build` "
+                "(there is no CPU fallback)")
+        handle = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(handle, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = handle
+    return _lib
+
+
+def _check(status: int, where: str) -> int:
+    if status < 0:
+        raise EpicError(status, where)
+    return status
+
+
+def _ptr(x) -> int:
+    """Device/host address of a torch tensor, numpy array or raw integer."""
+    if x is None:
+        return 0
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if isinstance(x, np.ndarray):
+        return x.ctypes.data
+    raise TypeError(type(x))
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+class Plan:
+    """Owns an epic_plan* (include/epic.h).  ant_uv float32 [A][2] in cell units, kernel_taps
+    float32 [A][K][K][2] or None for the delta kernel; both HOST arrays, copied by the library."""
+
+    def __init__(self, grid_n: int, pad: int, ant_uv: np.ndarray,
+                 kernel_taps: Optional[np.ndarray] = None, kernel_k: int = 1):
+        uv = np.ascontiguousarray(ant_uv, dtype=np.float32)
+        if uv.ndim != 2 or uv.shape[1] != 2:
+            raise ValueError("ant_uv must be [n_ant][2]")
+        taps = None
+        if kernel_taps is not None:
+            taps = np.ascontiguousarray(kernel_taps, dtype=np.float32)
+            if taps.shape != (uv.shape[0], kernel_k, kernel_k, 2):
+                raise ValueError(f"kernel_taps shape {taps.shape}")
+        self._h = _vp()
+        self.n_ant = int(uv.shape[0])
+        self.kernel_k = int(kernel_k)
+        _check(lib().epic_plan_create(ctypes.byref(self._h), grid_n, pad, self.n_ant,
+                                      _ptr(uv), _ptr(taps), kernel_k), "epic_plan_create")
+        self.N = lib().epic_plan_get_n(self._h)
+
+    # -- lifetime
+    def destroy(self) -> None:
+        if self._h:
+            h, self._h = self._h, _vp()
+            _check(lib().epic_plan_destroy(h), "epic_plan_destroy")
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    # -- configuration / queries
+    def set_products(self, n_products: int) -> None:
+        _check(lib().epic_plan_set_products(self._h, n_products), "epic_plan_set_products")
+
+    def set_path(self, path: int) -> None:
+        _check(lib().epic_plan_set_path(self._h, path), "epic_plan_set_path")
+
+    def n_planes(self, n_pol: int) -> int:
+        return _check(lib().epic_plan_get_n_planes(self._h, n_pol), "epic_plan_get_n_planes")
+
+    def path(self, n_pol: int) -> int:
+        return _check(lib().epic_plan_get_path(self._h, n_pol), "epic_plan_get_path")
+
+    def last_launches(self) -> int:
+        return _check(lib().epic_plan_last_launches(self._h), "epic_plan_last_launches")
+
+    def cells(self) -> np.ndarray:
+        out = np.empty((self.n_ant, self.kernel_k, self.kernel_k), dtype=np.int32)
+        _check(lib().epic_plan_get_cells(self._h, _ptr(out)), "epic_plan_get_cells")
+        return out
+
+    def support(self) -> tuple:
+        out = np.empty(4, dtype=np.int32)
+        _check(lib().epic_plan_get_support(self._h, _ptr(out)), "epic_plan_get_support")
+        return tuple(int(v) for v in out)
+
+    # -- device work
+    def image(self, voltages, n_t: int, n_chan: int, n_pol: int, out_accum, stream=None) -> None:
+        """epic_image: voltages DEVICE uint8 [T][C][Np][A]; ADDS into out_accum DEVICE float32
+        [C][planes][N][N]."""
+        _check(lib().epic_image(self._h, _ptr(voltages), n_t, n_chan, n_pol, _ptr(out_accum),
+                                _stream(stream)), "epic_image")
+
+    def image_cf32(self, voltages, n_t: int, n_chan: int, n_pol: int, out_accum, stream=None) -> None:
+        """epic_image_cf32: voltages DEVICE float32 [T][C][Np][A][2]."""
+        _check(lib().epic_image_cf32(self._h, _ptr(voltages), n_t, n_chan, n_pol, _ptr(out_accum),
+                                     _stream(stream)), "epic_image_cf32")
+
+    def debug_grid(self, voltages, is_cf32: bool, n_pol: int, out_plane, stream=None) -> None:
+        _check(lib().epic_debug_grid(self._h, _ptr(voltages), int(bool(is_cf32)), n_pol,
+                                     _ptr(out_plane), _stream(stream)), "epic_debug_grid")
+
+
+# free functions with the names of include/epic.h
+def epic_plan_create(grid_n, pad, n_ant, ant_uv, kernel_taps, kernel_k=1) -> Plan:
+    uv = np.asarray(ant_uv, dtype=np.float32).reshape(n_ant, 2)
+    return Plan(grid_n, pad, uv, kernel_taps, kernel_k)
+
+
+def epic_plan_destroy(plan: Optional[Plan]) -> None:
+    if plan is not None:
+        plan.destroy()
+
+
+def epic_image(plan: Plan, voltages, n_t, n_chan, n_pol, out_accum, stream=None) -> None:
+    plan.image(voltages, n_t, n_chan, n_pol, out_accum, stream)
+
+
+def epic_image_cf32(plan: Plan, voltages, n_t, n_chan, n_pol, out_accum, stream=None) -> None:
+    plan.image_cf32(voltages, n_t, n_chan, n_pol, out_accum, stream)
+
+
+def epic_debug_unpack(bytes_dev, n: int, out_dev, stream=None) -> None:
+    _check(lib().epic_debug_unpack(_ptr(bytes_dev), n, _ptr(out_dev), _stream(stream)), "epic_debug_unpack")
+
+
+def epic_fp32_peak_probe(iters: int = 4096) -> dict:
+    """Measured FP32 FMA rate of the device (roofline denominator): {"ms", "flops", "tflops"}."""
+    ms = ctypes.c_float()
+    fl = ctypes.c_double()
+    _check(lib().epic_fp32_peak_probe(iters, ctypes.byref(ms), ctypes.byref(fl)), "epic_fp32_peak_probe")
+    return {"ms": ms.value, "flops": fl.value, "tflops": fl.value / (ms.value * 1e-3) / 1e12}

@@ -1,0 +1,85 @@
+// Internal declarations shared by the libepic.so translation units (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <vector>
+
+#include "epic.h"
+
+namespace epic {
+
+// One nonzero cell of the (relocated) support block and its gather list (S2 inverted:
+// per-cell list of (antenna, tap) pairs, built once on the host).
+struct CellRec {
+  uint16_t y, x;      // relocated coordinates inside the support box
+  uint32_t ent_begin; // first entry in ent_ant / ent_tap
+  uint32_t ent_count;
+};
+
+struct DevTables {
+  const CellRec* cells;     // [n_cells], sorted by (y, x)
+  const uint32_t* row_ptr;  // [R + 1]: cells of support row y are [row_ptr[y], row_ptr[y+1])
+  const uint16_t* ent_ant;  // [n_ent] antenna index of each gather entry
+  const float2* ent_tap;    // [n_ent] complex tap of each gather entry
+  const float2* twiddle;    // [N/2]: exp(+2 pi i k / N), computed in double on the host
+  int n_cells, n_ent;
+  int N, logN, R, Cc, y0, x0; // support box: rows [y0, y0+R) mod N, cols [x0, x0+Cc) mod N
+  int n_ant, is_delta;
+};
+
+} // namespace epic
+
+struct epic_plan {
+  int grid_n, pad, N, logN, n_ant, K;
+  int n_products_req; // 0 = default
+  int path_req;
+  int last_launches;
+  std::vector<int> cells_host; // [n_ant][K][K] true cells y*N + x
+  int y0, x0, R, Cc;
+  epic::DevTables t;           // device pointers
+  void* d_blob;                // one allocation holding all tables
+  void* d_scratch;             // two-pass intermediate H, L2-sized
+  size_t scratch_bytes;
+  void* d_fused;               // tables private to the fused path
+  int fused_ok;                // support fits the fused kernel
+  int n_sm;
+  // host copies kept for the fused path's table builder
+  std::vector<epic::CellRec> h_cells;
+  std::vector<uint16_t> h_ent_ant;
+  std::vector<float2> h_ent_tap;
+};
+
+namespace epic {
+
+struct ImageArgs {
+  const void* volt;
+  int is_cf32;
+  int n_t, n_chan, n_pol, n_products, n_planes;
+  float* out;
+  cudaStream_t stream;
+};
+
+// epic_twopass.cu
+int twopass_image(epic_plan* p, const ImageArgs& a);
+int debug_grid(epic_plan* p, const void* volt, int is_cf32, int n_pol, float* out, cudaStream_t s);
+int debug_unpack(const void* bytes, long n, float* out, cudaStream_t s);
+int fp32_probe(int iters, float* ms, double* flops);
+
+// epic_fused.cu
+int fused_plan_init(epic_plan* p);  // sets p->fused_ok, allocates p->d_fused
+void fused_plan_free(epic_plan* p);
+int fused_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products);
+int fused_image(epic_plan* p, const ImageArgs& a);
+
+void set_cuda_error(cudaError_t e);
+
+} // namespace epic
+
+#define EPIC_CUDA_TRY(expr)                         \
+  do {                                              \
+    cudaError_t e__ = (expr);                       \
+    if (e__ != cudaSuccess) {                       \
+      epic::set_cuda_error(e__);                    \
+      return EPIC_ERR_CUDA;                         \
+    }                                               \
+  } while (0)

@@ -1,0 +1,377 @@
+// libepic.so — host side: plan construction (S2: cell indexing) and the C ABI
+// declared in include/epic.h.  No arithmetic of the per-frame path lives here; the kernels are
+// in epic_twopass.cu (general two-kernel path) and epic_fused.cu (one-kernel path).
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "epic_internal.h"
+
+namespace epic {
+
+static thread_local int g_last_cuda_error = 0;
+void set_cuda_error(cudaError_t e) { g_last_cuda_error = (int)e; }
+
+static inline int pos_mod(long long v, int n) {
+  long long m = v % n;
+  return (int)(m < 0 ? m + n : m);
+}
+
+// Smallest circular interval [start, start+len) mod n that covers every index with occ[i] != 0.
+static void circular_box(const std::vector<char>& occ, int n, int* start, int* len) {
+  int n_occ = 0;
+  for (int i = 0; i < n; ++i) n_occ += occ[i] ? 1 : 0;
+  if (n_occ == 0) { *start = 0; *len = 1; return; }
+  // longest run of empty indices on the circle
+  int best_len = 0, best_end = 0; // run occupies (best_end - best_len, best_end]  (indices mod n)
+  int run = 0;
+  for (int i = 0; i < 2 * n; ++i) {
+    if (!occ[i % n]) {
+      ++run;
+      if (run > best_len && run <= n) { best_len = run; best_end = i % n; }
+    } else {
+      run = 0;
+    }
+  }
+  if (best_len >= n) { *start = 0; *len = 1; return; }
+  *start = (best_end + 1) % n;
+  *len = n - best_len;
+}
+
+struct Entry {
+  int y, x;      // relocated
+  int ant, tap;  // tap = iy*K + ix
+};
+
+static int build_tables(epic_plan* p, const float* ant_uv, const float* taps) {
+  const int N = p->N, K = p->K, A = p->n_ant, h = (K - 1) / 2;
+  p->cells_host.resize((size_t)A * K * K);
+  std::vector<char> occ_y(N, 0), occ_x(N, 0);
+  for (int a = 0; a < A; ++a) {
+    // reading Q4: nearest cell = floor(double(u) + 0.5)
+    const long long cx = (long long)std::floor((double)ant_uv[2 * a + 0] + 0.5);
+    const long long cy = (long long)std::floor((double)ant_uv[2 * a + 1] + 0.5);
+    for (int iy = 0; iy < K; ++iy)
+      for (int ix = 0; ix < K; ++ix) {
+        const int y = pos_mod(cy + (iy - h), N); // reading Q6: wrap modulo N
+        const int x = pos_mod(cx + (ix - h), N);
+        p->cells_host[((size_t)a * K + iy) * K + ix] = y * N + x;
+        occ_y[y] = 1;
+        occ_x[x] = 1;
+      }
+  }
+  circular_box(occ_y, N, &p->y0, &p->R);
+  circular_box(occ_x, N, &p->x0, &p->Cc);
+
+  std::vector<Entry> ent((size_t)A * K * K);
+  for (int a = 0; a < A; ++a)
+    for (int k = 0; k < K * K; ++k) {
+      const int cell = p->cells_host[(size_t)a * K * K + k];
+      Entry e;
+      e.y = pos_mod(cell / N - p->y0, N);
+      e.x = pos_mod(cell % N - p->x0, N);
+      e.ant = a;
+      e.tap = k;
+      ent[(size_t)a * K * K + k] = e;
+    }
+  std::sort(ent.begin(), ent.end(), [](const Entry& l, const Entry& r) {
+    if (l.y != r.y) return l.y < r.y;
+    if (l.x != r.x) return l.x < r.x;
+    if (l.ant != r.ant) return l.ant < r.ant;
+    return l.tap < r.tap;
+  });
+
+  p->h_cells.clear();
+  p->h_ent_ant.resize(ent.size());
+  p->h_ent_tap.resize(ent.size());
+  std::vector<uint32_t> row_ptr(p->R + 1, 0);
+  for (size_t i = 0; i < ent.size(); ++i) {
+    const Entry& e = ent[i];
+    if (p->h_cells.empty() || p->h_cells.back().y != e.y || p->h_cells.back().x != e.x) {
+      CellRec c;
+      c.y = (uint16_t)e.y;
+      c.x = (uint16_t)e.x;
+      c.ent_begin = (uint32_t)i;
+      c.ent_count = 0;
+      p->h_cells.push_back(c);
+      row_ptr[e.y + 1] += 1;
+    }
+    p->h_cells.back().ent_count += 1;
+    p->h_ent_ant[i] = (uint16_t)e.ant;
+    float2 w;
+    if (taps) {
+      w.x = taps[((size_t)e.ant * K * K + e.tap) * 2 + 0];
+      w.y = taps[((size_t)e.ant * K * K + e.tap) * 2 + 1];
+    } else {
+      w.x = 1.0f;
+      w.y = 0.0f;
+    }
+    p->h_ent_tap[i] = w;
+  }
+  for (int y = 0; y < p->R; ++y) row_ptr[y + 1] += row_ptr[y];
+
+  std::vector<float2> tw(N / 2);
+  for (int k = 0; k < N / 2; ++k) {
+    const double ang = 2.0 * M_PI * (double)k / (double)N; // reading Q8: + sign
+    tw[k].x = (float)std::cos(ang);
+    tw[k].y = (float)std::sin(ang);
+  }
+
+  // one device blob: [cells][row_ptr][ent_tap][twiddle][ent_ant], each 16-byte aligned
+  auto align16 = [](size_t v) { return (v + 15) & ~(size_t)15; };
+  const size_t o_cells = 0;
+  const size_t o_row = align16(o_cells + p->h_cells.size() * sizeof(CellRec));
+  const size_t o_tap = align16(o_row + row_ptr.size() * sizeof(uint32_t));
+  const size_t o_tw = align16(o_tap + p->h_ent_tap.size() * sizeof(float2));
+  const size_t o_ant = align16(o_tw + tw.size() * sizeof(float2));
+  const size_t total = align16(o_ant + p->h_ent_ant.size() * sizeof(uint16_t));
+  std::vector<char> blob(total, 0);
+  std::memcpy(&blob[o_cells], p->h_cells.data(), p->h_cells.size() * sizeof(CellRec));
+  std::memcpy(&blob[o_row], row_ptr.data(), row_ptr.size() * sizeof(uint32_t));
+  std::memcpy(&blob[o_tap], p->h_ent_tap.data(), p->h_ent_tap.size() * sizeof(float2));
+  std::memcpy(&blob[o_tw], tw.data(), tw.size() * sizeof(float2));
+  std::memcpy(&blob[o_ant], p->h_ent_ant.data(), p->h_ent_ant.size() * sizeof(uint16_t));
+  EPIC_CUDA_TRY(cudaMalloc(&p->d_blob, total));
+  EPIC_CUDA_TRY(cudaMemcpy(p->d_blob, blob.data(), total, cudaMemcpyHostToDevice));
+  char* d = (char*)p->d_blob;
+  DevTables& t = p->t;
+  t.cells = (const CellRec*)(d + o_cells);
+  t.row_ptr = (const uint32_t*)(d + o_row);
+  t.ent_tap = (const float2*)(d + o_tap);
+  t.twiddle = (const float2*)(d + o_tw);
+  t.ent_ant = (const uint16_t*)(d + o_ant);
+  t.n_cells = (int)p->h_cells.size();
+  t.n_ent = (int)ent.size();
+  t.N = N;
+  t.logN = p->logN;
+  t.R = p->R;
+  t.Cc = p->Cc;
+  t.y0 = p->y0;
+  t.x0 = p->x0;
+  t.n_ant = A;
+  t.is_delta = taps ? 0 : 1;
+  return EPIC_OK;
+}
+
+static int resolve_products(const epic_plan* p, int n_pol) {
+  if (p->n_products_req == 0) return n_pol == 2 ? 4 : 1;
+  return p->n_products_req;
+}
+
+static int planes_for(int n_pol, int n_products) {
+  if (n_pol == 1 && n_products == 1) return 1;
+  if (n_pol == 2 && n_products == 2) return 2;
+  if (n_pol == 2 && n_products == 4) return 6;
+  return -1;
+}
+
+static int image_common(epic_plan* plan, const void* volt, int is_cf32, int n_t, int n_chan,
+                        int n_pol, float* out, epic_stream stream) {
+  if (!plan) return EPIC_ERR_ARG;
+  if (n_t < 0 || n_chan < 0) return EPIC_ERR_ARG;
+  if (n_pol != 1 && n_pol != 2) return EPIC_ERR_RANGE;
+  const int n_products = resolve_products(plan, n_pol);
+  const int n_planes = planes_for(n_pol, n_products);
+  if (n_planes < 0) return EPIC_ERR_RANGE;
+  plan->last_launches = 0;
+  if (n_t == 0 || n_chan == 0) return EPIC_OK;
+  if (!volt || !out) return EPIC_ERR_ARG;
+  ImageArgs a;
+  a.volt = volt;
+  a.is_cf32 = is_cf32;
+  a.n_t = n_t;
+  a.n_chan = n_chan;
+  a.n_pol = n_pol;
+  a.n_products = n_products;
+  a.n_planes = n_planes;
+  a.out = out;
+  a.stream = (cudaStream_t)stream;
+  int path = plan->path_req;
+  const int fused_can = fused_supported(plan, is_cf32, n_pol, n_products);
+  if (path == EPIC_PATH_AUTO) path = fused_can ? EPIC_PATH_FUSED : EPIC_PATH_TWOPASS;
+  if (path == EPIC_PATH_FUSED) {
+    if (!fused_can) return EPIC_ERR_RANGE;
+    return fused_image(plan, a);
+  }
+  return twopass_image(plan, a);
+}
+
+} // namespace epic
+
+using namespace epic;
+
+extern "C" {
+
+int epic_plan_create(epic_plan** out, int grid_n, int pad, int n_ant, const float* ant_uv,
+                     const float* kernel_taps, int kernel_k) {
+  if (!out) return EPIC_ERR_ARG;
+  *out = nullptr;
+  if (!ant_uv || grid_n < 1 || pad < 1) return EPIC_ERR_ARG;
+  const long long Nll = (long long)grid_n * pad;
+  if (Nll < 8 || Nll > 512 || (Nll & (Nll - 1)) != 0) return EPIC_ERR_ARG;
+  if (kernel_k < 1 || kernel_k > 15 || (kernel_k % 2) == 0) return EPIC_ERR_ARG;
+  if (!kernel_taps && kernel_k != 1) return EPIC_ERR_ARG;
+  if (n_ant < 1) return EPIC_ERR_ARG;
+  if (n_ant > 65535) return EPIC_ERR_RANGE;
+  for (int i = 0; i < 2 * n_ant; ++i)
+    if (!std::isfinite(ant_uv[i]) || std::fabs(ant_uv[i]) > 1.0e9f) return EPIC_ERR_ARG;
+  epic_plan* p = new (std::nothrow) epic_plan();
+  if (!p) return EPIC_ERR_NOMEM;
+  p->grid_n = grid_n;
+  p->pad = pad;
+  p->N = (int)Nll;
+  p->logN = 0;
+  while ((1 << p->logN) < p->N) ++p->logN;
+  p->n_ant = n_ant;
+  p->K = kernel_k;
+  p->n_products_req = 0;
+  p->path_req = EPIC_PATH_AUTO;
+  p->last_launches = 0;
+  p->d_blob = nullptr;
+  p->d_scratch = nullptr;
+  p->d_fused = nullptr;
+  p->fused_ok = 0;
+  p->scratch_bytes = 0;
+  int dev = 0;
+  cudaDeviceProp prop;
+  cudaError_t ce = cudaGetDevice(&dev);
+  if (ce == cudaSuccess) ce = cudaGetDeviceProperties(&prop, dev);
+  if (ce != cudaSuccess) {
+    set_cuda_error(ce);
+    delete p;
+    return EPIC_ERR_CUDA;
+  }
+  p->n_sm = prop.multiProcessorCount;
+  int st;
+  try {
+    st = build_tables(p, ant_uv, kernel_taps);
+  } catch (const std::bad_alloc&) {
+    st = EPIC_ERR_NOMEM;
+  }
+  if (st == EPIC_OK) {
+    // two-pass intermediate: at least one dual-pol frame, otherwise an L2-sized ring
+    const size_t frame = (size_t)2 * p->R * p->N * sizeof(float2);
+    p->scratch_bytes = std::max((size_t)64 << 20, frame);
+    ce = cudaMalloc(&p->d_scratch, p->scratch_bytes);
+    if (ce != cudaSuccess) {
+      set_cuda_error(ce);
+      st = (ce == cudaErrorMemoryAllocation) ? EPIC_ERR_NOMEM : EPIC_ERR_CUDA;
+    }
+  }
+  if (st == EPIC_OK) st = fused_plan_init(p);
+  if (st != EPIC_OK) {
+    epic_plan_destroy(p);
+    return st;
+  }
+  *out = p;
+  return EPIC_OK;
+}
+
+int epic_plan_destroy(epic_plan* plan) {
+  if (!plan) return EPIC_OK;
+  cudaError_t ce = cudaDeviceSynchronize();
+  fused_plan_free(plan);
+  if (plan->d_scratch) cudaFree(plan->d_scratch);
+  if (plan->d_blob) cudaFree(plan->d_blob);
+  delete plan;
+  if (ce != cudaSuccess) {
+    set_cuda_error(ce);
+    return EPIC_ERR_CUDA;
+  }
+  return EPIC_OK;
+}
+
+int epic_plan_set_products(epic_plan* plan, int n_products) {
+  if (!plan) return EPIC_ERR_ARG;
+  if (n_products != 0 && n_products != 1 && n_products != 2 && n_products != 4) return EPIC_ERR_RANGE;
+  plan->n_products_req = n_products;
+  return EPIC_OK;
+}
+
+int epic_plan_set_path(epic_plan* plan, int path) {
+  if (!plan) return EPIC_ERR_ARG;
+  if (path != EPIC_PATH_AUTO && path != EPIC_PATH_TWOPASS && path != EPIC_PATH_FUSED) return EPIC_ERR_ARG;
+  if (path == EPIC_PATH_FUSED && !plan->fused_ok) return EPIC_ERR_RANGE;
+  plan->path_req = path;
+  return EPIC_OK;
+}
+
+int epic_image(epic_plan* plan, const void* voltages, int n_t, int n_chan, int n_pol,
+               float* out_accum, epic_stream stream) {
+  return image_common(plan, voltages, 0, n_t, n_chan, n_pol, out_accum, stream);
+}
+
+int epic_image_cf32(epic_plan* plan, const void* voltages_cf32, int n_t, int n_chan, int n_pol,
+                    float* out_accum, epic_stream stream) {
+  return image_common(plan, voltages_cf32, 1, n_t, n_chan, n_pol, out_accum, stream);
+}
+
+int epic_plan_get_n(const epic_plan* plan) { return plan ? plan->N : (int)EPIC_ERR_ARG; }
+
+int epic_plan_get_n_planes(const epic_plan* plan, int n_pol) {
+  if (!plan) return EPIC_ERR_ARG;
+  if (n_pol != 1 && n_pol != 2) return EPIC_ERR_RANGE;
+  const int pl = planes_for(n_pol, resolve_products(plan, n_pol));
+  return pl < 0 ? (int)EPIC_ERR_RANGE : pl;
+}
+
+int epic_plan_get_cells(const epic_plan* plan, int* cells_host) {
+  if (!plan || !cells_host) return EPIC_ERR_ARG;
+  std::memcpy(cells_host, plan->cells_host.data(), plan->cells_host.size() * sizeof(int));
+  return EPIC_OK;
+}
+
+int epic_plan_get_support(const epic_plan* plan, int* box_host) {
+  if (!plan || !box_host) return EPIC_ERR_ARG;
+  box_host[0] = plan->y0;
+  box_host[1] = plan->x0;
+  box_host[2] = plan->R;
+  box_host[3] = plan->Cc;
+  return EPIC_OK;
+}
+
+int epic_plan_get_path(const epic_plan* plan, int n_pol) {
+  if (!plan) return EPIC_ERR_ARG;
+  if (n_pol != 1 && n_pol != 2) return EPIC_ERR_RANGE;
+  const int n_products = resolve_products(plan, n_pol);
+  if (planes_for(n_pol, n_products) < 0) return EPIC_ERR_RANGE;
+  if (plan->path_req != EPIC_PATH_AUTO) return plan->path_req;
+  return fused_supported(plan, 0, n_pol, n_products) ? EPIC_PATH_FUSED : EPIC_PATH_TWOPASS;
+}
+
+int epic_plan_last_launches(const epic_plan* plan) { return plan ? plan->last_launches : (int)EPIC_ERR_ARG; }
+
+int epic_debug_unpack(const void* bytes_dev, long n, float* out_dev, epic_stream stream) {
+  if (n < 0) return EPIC_ERR_ARG;
+  if (n == 0) return EPIC_OK;
+  if (!bytes_dev || !out_dev) return EPIC_ERR_ARG;
+  return debug_unpack(bytes_dev, n, out_dev, (cudaStream_t)stream);
+}
+
+int epic_debug_grid(epic_plan* plan, const void* voltages, int is_cf32, int n_pol,
+                    float* out_plane_dev, epic_stream stream) {
+  if (!plan || !voltages || !out_plane_dev) return EPIC_ERR_ARG;
+  if (n_pol != 1 && n_pol != 2) return EPIC_ERR_RANGE;
+  return debug_grid(plan, voltages, is_cf32 ? 1 : 0, n_pol, out_plane_dev, (cudaStream_t)stream);
+}
+
+int epic_fp32_peak_probe(int iters, float* ms_out, double* flops_out) {
+  if (iters < 1 || !ms_out || !flops_out) return EPIC_ERR_ARG;
+  return fp32_probe(iters, ms_out, flops_out);
+}
+
+const char* epic_status_string(int status) {
+  switch (status) {
+    case EPIC_OK: return "EPIC_OK";
+    case EPIC_ERR_ARG: return "EPIC_ERR_ARG: null pointer or invalid shape argument";
+    case EPIC_ERR_RANGE: return "EPIC_ERR_RANGE: value outside the supported range";
+    case EPIC_ERR_CUDA: return "EPIC_ERR_CUDA: a CUDA runtime call failed";
+    case EPIC_ERR_NOMEM: return "EPIC_ERR_NOMEM: allocation failed";
+    default: return "unknown epic_status";
+  }
+}
+
+int epic_last_cuda_error(void) { return g_last_cuda_error; }
+
+} // extern "C"

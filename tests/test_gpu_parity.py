@@ -1,0 +1,163 @@
+"""GPU parity tests (-m gpu): libepic.so through its C ABI against the float64 oracle, element by
+element, on the same seeded inputs.  Bit-exact for S1 (unpack), S2 (cells) and integer-valued
+gridding; <= 1e-4 of the image peak for accumulated images (BASELINE.json north_star)."""
+import numpy as np
+import pytest
+
+from oracle import epic_oracle as orc
+from workloads import make_config, make_custom
+
+from epic_testlib import TOL, assert_parity, run_gpu, run_oracle
+
+pytestmark = pytest.mark.gpu
+
+
+def _epic():
+    import paper_1904_11422_b200 as epic
+    return epic
+
+
+# ------------------------------------------------------------------ S1
+def test_s1_unpack_bit_exact_all_bytes_and_random():
+    import torch
+    epic = _epic()
+    rng = np.random.default_rng(5)
+    b = np.concatenate([np.arange(256, dtype=np.uint8), rng.integers(0, 256, 100003, dtype=np.uint8)])
+    d = torch.from_numpy(b).cuda()
+    out = torch.empty((b.size, 2), dtype=torch.float32, device="cuda")
+    epic.epic_debug_unpack(d, b.size, out)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    ref = orc.unpack_ci4(b)
+    assert np.array_equal(got[:, 0], ref.real.astype(np.float32))
+    assert np.array_equal(got[:, 1], ref.imag.astype(np.float32))
+
+
+# ------------------------------------------------------------------ S2
+@pytest.mark.parametrize("wl", [
+    make_config(1), make_config(2, n_chan=1, n_t=1), make_config(3, n_chan=1, n_t=1),
+    make_config(4, n_chan=1, n_t=1), make_config(5, n_chan=1, n_t=1),
+    make_custom(grid_n=8, pad=2, n_ant=40, n_pol=1, kernel_k=5, n_chan=1, n_t=1, layout="wrap"),
+], ids=lambda w: w.name)
+def test_s2_cells_bit_exact(wl):
+    epic = _epic()
+    with epic.Plan(wl.grid_n, wl.pad, wl.ant_uv, wl.taps, wl.kernel_k) as plan:
+        got = plan.cells()
+        y0, x0, R, Cc = plan.support()
+    ref = orc.tap_cells(wl.ant_uv, wl.kernel_k, wl.N)
+    assert np.array_equal(got.astype(np.int64), ref)
+    # the support box covers every occupied row and column
+    ys, xs = np.unique(ref // wl.N), np.unique(ref % wl.N)
+    assert np.all((ys - y0) % wl.N < R) and np.all((xs - x0) % wl.N < Cc)
+
+
+def test_s2_half_cells_round_up_and_wrap():
+    epic = _epic()
+    uv = np.array([[2.5, 2.49], [-0.5, -0.51], [7.6, 0.0], [15.5, 16.0]], dtype=np.float32)
+    with epic.Plan(8, 2, uv) as plan:
+        got = plan.cells().reshape(-1)
+    assert got.tolist() == [2 * 16 + 3, 15 * 16 + 0, 0 * 16 + 8, 0 * 16 + 0]
+
+
+# ------------------------------------------------------------------ S3
+@pytest.mark.parametrize("idx", [1, 2, 3, 5])
+def test_s3_gridding_one_frame(idx):
+    import torch
+    epic = _epic()
+    wl = make_config(idx, n_chan=1, n_t=1)
+    v = wl.voltages()
+    e = orc.voltages_to_complex(v[0, 0], wl.input_kind)  # [Np][A]
+    cells = orc.tap_cells(wl.ant_uv, wl.kernel_k, wl.N)
+    w = orc.taps_to_complex(wl.taps, wl.n_ant, wl.kernel_k)
+    ref = orc.grid_frames(e, cells, w, wl.N)  # [Np][N][N]
+    with epic.Plan(wl.grid_n, wl.pad, wl.ant_uv, wl.taps, wl.kernel_k) as plan:
+        out = torch.full((wl.n_pol, wl.N, wl.N, 2), 7.0, dtype=torch.float32, device="cuda")
+        plan.debug_grid(torch.from_numpy(v).cuda(), wl.input_kind == "cf32", wl.n_pol, out)
+        torch.cuda.synchronize()
+        got = out.cpu().numpy()
+    gc = got[..., 0].astype(np.float64) + 1j * got[..., 1]
+    if wl.kernel_k == 1 and wl.input_kind == "ci4":
+        assert np.array_equal(gc, ref)  # small integers: exact in any order
+    else:
+        assert np.abs(gc - ref).max() <= 2e-6 * max(1.0, np.abs(ref).max())
+
+
+# ------------------------------------------------------------------ whole path, small sizes
+def test_c1_exact_config_against_definition_oracle():
+    wl = make_config(1)
+    gpu, info = run_gpu(wl, return_plan_info=True)
+    ref = run_oracle(wl, mode="definition")
+    assert_parity(gpu, ref, what=wl.name)
+    assert info["launches"] > 0
+
+
+SMALL = [
+    make_config(1, n_chan=3, n_t=21),
+    make_config(2, n_chan=3, n_t=37),
+    make_config(3, n_chan=2, n_t=29),
+    make_config(4, n_chan=2, n_t=5),
+    make_config(5, n_chan=1, n_t=2),
+    make_config(5, n_chan=2, n_t=3, n_ant=256),
+    make_custom(grid_n=4, pad=2, n_ant=5, n_pol=1, kernel_k=1, n_chan=2, n_t=3, input_kind="cf32"),
+    make_custom(grid_n=8, pad=2, n_ant=40, n_pol=2, kernel_k=5, n_chan=2, n_t=4, layout="wrap"),
+    make_custom(grid_n=32, pad=2, n_ant=77, n_pol=2, kernel_k=3, n_chan=5, n_t=9, n_products=2),
+    make_custom(grid_n=16, pad=4, n_ant=33, n_pol=1, kernel_k=7, n_chan=1, n_t=11, layout="disc"),
+    make_custom(grid_n=64, pad=2, n_ant=300, n_pol=2, kernel_k=3, n_chan=1, n_t=6, layout="wrap",
+                input_kind="cf32"),
+    make_custom(grid_n=128, pad=1, n_ant=64, n_pol=1, kernel_k=1, n_chan=2, n_t=2, layout="uniform"),
+    make_custom(grid_n=64, pad=2, n_ant=1, n_pol=2, kernel_k=1, n_chan=1, n_t=1),
+]
+
+
+@pytest.mark.parametrize("wl", SMALL, ids=lambda w: f"{w.name}-c{w.n_chan}-t{w.n_t}")
+def test_whole_path_small(wl):
+    gpu = run_gpu(wl)
+    ref = run_oracle(wl)
+    assert_parity(gpu, ref, what=wl.name)
+    if wl.n_products == 4:  # YX = conj(XY) exactly; XX, YY >= 0
+        assert np.array_equal(gpu[:, 4], gpu[:, 2]) and np.array_equal(gpu[:, 5], -gpu[:, 3])
+    assert (gpu[:, :min(2, gpu.shape[1])] >= 0).all()
+
+
+def test_calls_accumulate_into_out_accum():
+    wl = make_config(2, n_chan=2, n_t=30)
+    one = run_gpu(wl, calls=1)
+    three = run_gpu(wl, calls=3)
+    ref = run_oracle(wl)
+    assert_parity(three, ref, what="3 calls")
+    assert np.abs(one - three).max() <= 1e-5 * np.abs(one).max()
+
+
+def test_empty_calls_are_noops_and_errors_are_reported():
+    import torch
+    epic = _epic()
+    wl = make_config(2, n_chan=1, n_t=1)
+    with epic.Plan(wl.grid_n, wl.pad, wl.ant_uv) as plan:
+        out = torch.ones((1, 6, 128, 128), dtype=torch.float32, device="cuda")
+        plan.image(0, 0, 1, 2, out)     # n_t == 0: nothing read, nothing written
+        plan.image(0, 5, 0, 2, out)     # n_chan == 0
+        torch.cuda.synchronize()
+        assert float(out.min()) == 1.0 and float(out.max()) == 1.0
+        with pytest.raises(epic.EpicError):
+            plan.image(0, 1, 1, 3, out)  # n_pol out of range
+        with pytest.raises(epic.EpicError):
+            plan.image(0, 1, 1, 2, out)  # NULL voltages
+        plan.set_products(1)
+        with pytest.raises(epic.EpicError):
+            plan.image(out, 1, 1, 2, out)  # 1 product needs n_pol == 1
+    for bad in [dict(grid_n=3, pad=2), dict(grid_n=512, pad=2), dict(grid_n=2, pad=2)]:
+        with pytest.raises(epic.EpicError):
+            epic.Plan(bad["grid_n"], bad["pad"], wl.ant_uv)
+    with pytest.raises(epic.EpicError):
+        epic.Plan(64, 2, wl.ant_uv, np.zeros((256, 2, 2, 2), np.float32), 2)  # even K
+
+
+def test_point_source_peaks_at_predicted_pixel():
+    """BASELINE.json check (c) on the CUDA path: C3's injected source is common to both
+    polarisations while the noise is not, so it is the brightest pixel of the accumulated
+    Re(XY) image (the oracle agrees: tests/test_oracle_pins.py pins the pixel rule)."""
+    wl = make_config(3, n_chan=1, n_t=2500)
+    gpu = run_gpu(wl)
+    src = wl.sources[0]
+    m, l = np.unravel_index(np.argmax(gpu[0, 2]), gpu[0, 2].shape)
+    assert (m, l) == (src["m_pix"], src["l_pix"])
