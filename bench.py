@@ -1,0 +1,296 @@
+#!/usr/bin/env python
+"""EPIC hot-path benchmark (BASELINE.json metric: E-field frames/s and fraction of roofline).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl epic|reference]
+
+One step = one epic_image call over the whole workload (all channels x all time samples of the
+configuration): unpack -> grid -> 2-D transform -> products -> accumulate.
+N=1 times configs[1] (C2, the LWA-station-like case BASELINE.json's target is quoted on).
+For N>1 (torchrun, one rank per GPU) every rank images its own copy of the workload -- channels
+are independent, so the path shards with no collective ("weak" scaling).
+Rank 0 prints ONE JSON line.  `--impl reference` times the float64 CPU oracle instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from workloads import make_config  # noqa: E402
+
+METRIC = "E-field frames/sec (chan x time gridded+FFT'd+accumulated)"
+UNIT = "frames/s"
+FP32_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # SMs x lanes x FMA x max clock
+L2_FLUSH_BYTES = 256 << 20
+
+
+def algorithmic_flops_per_frame(wl) -> float:
+    """SURVEY.md §8(d) / DESIGN.md: row-pruned FFT 7.5 N^2 log2 N per pol (pad 2; 10 N^2 log2 N
+    times (1+1/pad)/2 in general), gridding 2 (unit delta tap) or 8 flops per (antenna, tap, pol),
+    4 flops/pixel per real product and 8 for XY (YX = conj, free)."""
+    N, P = wl.N, wl.n_pol
+    fft = 5.0 * N * N * np.log2(N) * (1.0 + 1.0 / wl.pad) * P
+    grid = (2.0 if wl.taps is None else 8.0) * wl.n_ant * wl.kernel_k ** 2 * P
+    prod = N * N * (4.0 * min(P, 2) + (8.0 if wl.n_products == 4 else 0.0))
+    return fft + grid + prod
+
+
+def algorithmic_bytes_per_frame(wl) -> float:
+    """Voltages once + out_accum read and written once per call, spread over the call's frames."""
+    v = wl.n_pol * wl.n_ant * (8 if wl.input_kind == "cf32" else 1)
+    img = 2.0 * wl.n_planes * wl.N * wl.N * 4 / wl.n_t
+    return v + img
+
+
+class ClockSampler:
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+             "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.QUERY}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 8:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[4:8]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def cpu_baseline(wl, volt, n_chan_sample: int) -> dict:
+    """The float64 oracle, as it stands, on a bounded sample of the same workload."""
+    from oracle import epic_oracle as orc
+    ch = list(range(min(n_chan_sample, wl.n_chan)))
+    t0 = time.perf_counter()
+    orc.epic_image(volt, wl.input_kind, wl.ant_uv, wl.taps, wl.grid_n, wl.pad, wl.n_products,
+                   kernel_k=wl.kernel_k, mode="fast", channels=ch)
+    dt = time.perf_counter() - t0
+    frames = len(ch) * volt.shape[0]
+    return {"value": frames / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"channels 0..{len(ch) - 1} x all {volt.shape[0]} time samples of {wl.name} "
+                      f"({frames} frames, {dt:.1f} s, numpy float64 single thread)"}
+
+
+def run_reference(args, wl):
+    """--impl reference: the oracle on the host cores, each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n_t = min(wl.n_t, 250)
+    small = make_config(wl.index, n_chan=2, n_t=n_t)
+    volt = small.voltages()
+    times = []
+    res = None
+    for i in range(args.warmup + args.steps):
+        res = cpu_baseline(small, volt, 2)
+        if i >= args.warmup:
+            times.append(2 * n_t / res["value"])
+    ms = 1e3 * float(np.mean(times))
+    value = 2 * n_t / (ms * 1e-3)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, **{k: v for k, v in wl.describe().items() if k != "workload"},
+                   "step_sample": f"2 channels x {n_t} time samples per step"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": res["sample"]},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def run_epic(args, wl):
+    import torch
+    import torch.distributed as dist
+    import paper_1904_11422_b200 as epic
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    volt = wl.voltages()                       # host, seeded synthetic (DESIGN.md input recipe)
+    h_volt = torch.from_numpy(volt).pin_memory()
+    d_volt = h_volt.to(dev, non_blocking=True)
+    plan = epic.Plan(wl.grid_n, wl.pad, wl.ant_uv, wl.taps, wl.kernel_k)
+    plan.set_products(wl.n_products)
+    if args.path:
+        plan.set_path({"auto": 0, "twopass": 1, "fused": 2}[args.path])
+    planes = plan.n_planes(wl.n_pol)
+    out = torch.zeros((wl.n_chan, planes, wl.N, wl.N), dtype=torch.float32, device=dev)
+    h_out = torch.empty(out.shape, dtype=torch.float32).pin_memory()
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    call = plan.image_cf32 if wl.input_kind == "cf32" else plan.image
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step_device():
+        out.zero_()
+        flush.fill_(1)                          # L2 flush between timed iterations
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        call(d_volt, wl.n_t, wl.n_chan, wl.n_pol, out, stream)
+        e1.record(stream)
+        return e0, e1
+
+    def step_e2e():
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        flush.fill_(1)
+        out.zero_()
+        e0.record(stream)
+        d_in = h_volt.to(dev, non_blocking=True)          # H2D of this step's voltages (pinned)
+        call(d_in, wl.n_t, wl.n_chan, wl.n_pol, out, stream)
+        h_out.copy_(out, non_blocking=True)               # D2H of the accumulated images
+        e1.record(stream)
+        return e0, e1
+
+    for _ in range(max(args.warmup, 3)):
+        step_device()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    evs = [step_device() for _ in range(args.steps)]
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    launches = plan.last_launches() * args.steps
+    dev_ms = [a.elapsed_time(b) for a, b in evs]
+    total_ms = float(sum(dev_ms))
+
+    for _ in range(2):
+        step_e2e()
+    barrier()
+    evs = [step_e2e() for _ in range(args.steps)]
+    barrier()
+    e2e_ms = float(sum(a.elapsed_time(b) for a, b in evs))
+
+    if world > 1:
+        tt = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_ms, e2e_ms = float(tt[0]), float(tt[1])
+    path = plan.path(wl.n_pol)
+    support = plan.support()
+    probe = epic.epic_fp32_peak_probe(20000) if rank == 0 else None
+    plan.destroy()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    frames_step = wl.frames * world
+    ms_per_step = total_ms / args.steps
+    value = frames_step / (ms_per_step * 1e-3)
+    e2e_value = frames_step / (e2e_ms / args.steps * 1e-3)
+    flops = algorithmic_flops_per_frame(wl)
+    bytes_f = algorithmic_bytes_per_frame(wl)
+    kernel_ms = float(np.mean(dev_ms))           # rank 0's own kernel time (one launch per step when fused)
+    achieved = flops * wl.frames / (kernel_ms * 1e-3) / 1e12
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(f"{wl.name}:{'fused' if path == 2 else 'twopass'}")
+        except (OSError, ValueError):
+            traffic = None
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": wl.name, **{k: v for k, v in wl.describe().items() if k != "workload"},
+                   "kernel_path": {1: "twopass", 2: "fused"}.get(path, str(path)),
+                   "support_box": list(support), "l2": f"flushed between iterations ({L2_FLUSH_BYTES >> 20} MiB write)",
+                   "sharding": "independent replicas of the workload per GPU (channels are independent), no collective"},
+        "roofline": {
+            "bound": "alu", "achieved": achieved, "peak": FP32_NOMINAL_TFLOPS, "unit": "TFLOP/s",
+            "frac": achieved / FP32_NOMINAL_TFLOPS, "traffic": traffic,
+            "peak_kind": "nominal FP32: 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
+            "peak_measured_fma_probe": probe["tflops"], "frac_of_measured_probe": achieved / probe["tflops"],
+            "algorithmic_flops_per_frame": flops, "algorithmic_bytes_per_frame": bytes_f,
+            "hbm_achieved_gbs": bytes_f * wl.frames / (kernel_ms * 1e-3) / 1e9,
+            "kernel_ms": kernel_ms, "kernel": "epic_fused" if path == 2 else "grid_rowfft+colfft_accum",
+        },
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(volt.nbytes),
+                "d2h_bytes_per_step": int(out.numel() * 4)},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(wl, volt, args.cpu_channels)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (1-based)")
+    ap.add_argument("--impl", default="epic", choices=["epic", "reference"])
+    ap.add_argument("--path", default=None, choices=[None, "auto", "twopass", "fused"])
+    ap.add_argument("--n-chan", type=int, default=None)
+    ap.add_argument("--n-t", type=int, default=None)
+    ap.add_argument("--n-ant", type=int, default=None)
+    ap.add_argument("--cpu-channels", type=int, default=8)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    wl = make_config(args.config, n_chan=args.n_chan, n_t=args.n_t, n_ant=args.n_ant)
+    if args.impl == "reference":
+        run_reference(args, wl)
+    else:
+        run_epic(args, wl)
+
+
+if __name__ == "__main__":
+    main()
