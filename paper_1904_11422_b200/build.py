@@ -19,7 +19,7 @@ SOURCES = ["epic_plan.cu", "epic_twopass.cu", "epic_fused.cu"]
 HEADERS = [os.path.join(CSRC, "epic_internal.h"), os.path.join(ROOT, "include", "epic.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--use_fast_math=false",
+    "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--use_fast_math=false", "--expt-relaxed-constexpr",
 ]
 
 
