@@ -1,32 +1,40 @@
-// Fused EPIC path: unpack -> grid -> 2-D transform -> products -> accumulate in ONE kernel, the
+// Fused EPIC path: unpack -> grid -> 2-D transform -> products -> accumulate in ONE kernel; the
 // aperture/image planes never leave the SM (BASELINE.json north_star (1)-(4)).
 //
 // Applies when the occupied cells of the aperture fit a 32 x 32 box (after the circular
-// relocation of epic_plan.cu; SURVEY.md reading Q7) and N = 32*Q, Q in {1,2,4,8}.  With the
-// support S = 32 cells a side, the N x N image splits into Q*Q independent 32 x 32 sub-images
+// relocation of epic_plan.cu; reading Q7) and N = 32*Q, Q in {2,4}.  With the support
+// S = 32 cells a side the N x N image splits into Q*Q independent 32 x 32 sub-images
 //
 //   A[Q m1 + m2][Q l1 + l2] = sum_{y,x<32} G[y][x] W_N^{x l2} W_N^{y m2} W_32^{x l1 + y m1},
 //
-// i.e. the zero rows/columns of the padded plane are never transformed (a pruned decimation-in-
-// frequency 2-D FFT: the first log2 Q stages of each axis only multiply by a phase ramp).
+// so the structurally-zero rows/columns of the padded plane are never transformed (a pruned
+// decimation-in-frequency 2-D FFT whose first log2 Q stages per axis are phase ramps).
+//
+// Packing.  Every complex value is carried as a PAIR of planes in the two halves of f32x2
+// registers (sm_100 FFMA2/FADD2/FMUL2: one issue slot, two FP32 lanes): (lo, hi) = (pol X, pol Y)
+// of one time sample when n_pol == 2, or two consecutive time samples when n_pol == 1.  Both
+// halves see the same twiddles, so the whole transform is packed arithmetic; a shared-memory
+// cell is a float4 (re_lo, re_hi, im_lo, im_hi).
+//
 // Work unit = (channel c, column residue l2); its CTA owns the image columns l = Q l1 + l2 and
-// keeps their accumulators in registers for the whole integration:
+// keeps their accumulators in registers for the unit's whole time range.  One 32-point transform
+// with ramp is split over two threads h = 0,1 (outputs 2k + h):
 //
-//   per batch of Q frames:
-//     stage    cp.async the next batch's 4+4-bit voltages into shared memory (double buffer)
-//     gather   S1+S3: every thread owns fixed cells of the 32x32 block and sums its (antenna, tap)
-//              list in table order (no atomics, deterministic) for all frames/pols of the batch
-//     rows     S4 along x: one thread per (frame, pol, row): 32 inputs -> the 32 outputs l1 of
-//              this CTA's l2, in registers, written back in place
-//     columns  S4 along y + S5 + S6: one thread per (pol, m2, l1): 32 inputs from shared memory ->
-//              32 outputs m1 in registers -> products -> += register accumulators
-//   at the end of the unit's frames: one atomicAdd per pixel into out_accum.
+//   X[2Q k + rho] = sum_{y<16} [ (in[y] + (-1)^h in[y+16]) W_N^{y rho} ] W_16^{y k},  rho = r + Q h,
 //
-// The 32-point transforms run as TWO 16-point FFTs packed in the halves of f32x2 registers
-// (sm_100 FFMA2/FADD2): outputs 2Q k + rho for rho = m2 (low half) and m2 + Q (high half),
-// k = 0..15, of   X[2Q k + rho] = sum_{y<16} (in[y] W_N^{y rho} + in[y+16] W_N^{(y+16) rho}) W_16^{y k}.
-// The bracket ("fold + ramp") is scalar FP32 with compile-time twiddles; the 16-point FFT is
-// radix-2 decimation-in-time with the 6-FMA butterfly, twiddles as immediates.
+// i.e. fold, multiply by a table twiddle, 16-point radix-2 FFT with immediate twiddles.  Rows
+// (along x, r = l2) and columns (along y, r = m2) run the SAME code, so the hot loop is a few KB
+// of instructions shared by all warps (the first version of this kernel unrolled every residue
+// separately, 109 KB of code, and was instruction-fetch bound: profiles/r01_fused_v1_*).
+//
+//   per batch of F pairs (F time samples when n_pol == 2):
+//     prefetch  next batch's 4+4-bit voltages, global -> registers (consumed one batch later)
+//     gather    S3: every thread owns fixed cells of the 32x32 block and sums its (antenna, tap)
+//               list in table order from the unpacked voltages E (no atomics, deterministic)
+//     rows      S4 along x, thread = (pair, row y, h), in place
+//     unpack    S1: the prefetched words -> E (float4 per antenna) for the NEXT batch
+//     columns   S4 along y + S5 + S6: thread = (l1, rho); 16 outputs -> products -> += registers
+//   at the end of the unit's time range: one add per pixel into out_accum.
 #include <algorithm>
 
 #include "epic_internal.h"
@@ -34,8 +42,12 @@
 namespace epic {
 namespace {
 
-constexpr int S = 32;   // support block side (cells)
-constexpr int HS = 34;  // row stride of the shared planes, complex elements (16-byte rows, conflict-free)
+constexpr int S = 32;        // support block side (cells)
+constexpr int HS = 34;       // row stride of a shared plane in float4 cells (bank-conflict-free)
+constexpr int PLANE = S * HS;  // float4 cells per pair-plane
+constexpr int F = 4;         // pairs per batch
+constexpr int MAXW = 2;      // prefetched word pairs per thread
+constexpr int CHUNK = 2;     // fold_ramp: elements whose loads may be in flight together
 
 // ---------------------------------------------------------------- compile-time twiddles
 // exp(+2 pi i ex / n) in double, evaluated by the compiler (reading Q8: + sign, inverse DFT).
@@ -70,40 +82,10 @@ constexpr double tw_sin(int ex, int n) {
 constexpr int bitrev4(int v) { return ((v & 1) << 3) | ((v & 2) << 1) | ((v & 4) >> 1) | ((v & 8) >> 3); }
 
 // ---------------------------------------------------------------- packed complex pair
-// (lo, hi) halves hold two independent 16-point transforms (rho = r and r + Q).
-struct C2 { float2 re, im; };
+struct C2 { float2 re, im; };  // (lo, hi) halves = two independent planes
 
 __device__ __forceinline__ float2 f2(float v) { return make_float2(v, v); }
 __device__ __forceinline__ float2 neg2(float2 v) { return make_float2(-v.x, -v.y); }
-
-// acc += v * exp(2 pi i EX / NN), scalar, compile-time twiddle
-template <int EX, int NN>
-__device__ __forceinline__ void cmadd(float& ar, float& ai, float vr, float vi) {
-  constexpr int e = mod_pos(EX, NN);
-  if constexpr (e == 0) { ar += vr; ai += vi; }
-  else if constexpr (4 * e == NN) { ar -= vi; ai += vr; }
-  else if constexpr (2 * e == NN) { ar -= vr; ai -= vi; }
-  else if constexpr (4 * e == 3 * NN) { ar += vi; ai -= vr; }
-  else {
-    constexpr float wr = (float)tw_cos(e, NN), wi = (float)tw_sin(e, NN);
-    ar = fmaf(vr, wr, ar); ar = fmaf(-vi, wi, ar);
-    ai = fmaf(vi, wr, ai); ai = fmaf(vr, wi, ai);
-  }
-}
-// v * exp(2 pi i EX / NN)
-template <int EX, int NN>
-__device__ __forceinline__ void cmul_tw(float& outr, float& outi, float vr, float vi) {
-  constexpr int e = mod_pos(EX, NN);
-  if constexpr (e == 0) { outr = vr; outi = vi; }
-  else if constexpr (4 * e == NN) { outr = -vi; outi = vr; }
-  else if constexpr (2 * e == NN) { outr = -vr; outi = -vi; }
-  else if constexpr (4 * e == 3 * NN) { outr = vi; outi = -vr; }
-  else {
-    constexpr float wr = (float)tw_cos(e, NN), wi = (float)tw_sin(e, NN);
-    outr = fmaf(-vi, wi, vr * wr);
-    outi = fmaf(vr, wi, vi * wr);
-  }
-}
 
 // radix-2 DIT butterfly on packed pairs: (a, b) <- (a + w b, a - w b), w = exp(2 pi i K / NN)
 template <int K, int NN>
@@ -126,7 +108,6 @@ __device__ __forceinline__ void bfly(C2& a, C2& b) {
     a = p;
   }
 }
-
 template <int NN, int BASE, int K>
 __device__ __forceinline__ void fft16_block(C2 (&z)[16]) {
   if constexpr (K < NN / 2) {
@@ -149,38 +130,36 @@ __device__ __forceinline__ void fft16(C2 (&z)[16]) {
   fft16_stage<16, 0>(z);
 }
 
-// fold + ramp for input pair (y, y+16) of residue pair (RHO, RHO+Q), N = 32 Q
-template <int Q, int RHO, int Y>
-__device__ __forceinline__ void fold_one(C2 (&z)[16], float2 a, float2 b, bool has_b) {
-  constexpr int N = 32 * Q;
-  float lr, li, hr, hi;
-  cmul_tw<Y * RHO, N>(lr, li, a.x, a.y);
-  cmul_tw<Y * (RHO + Q), N>(hr, hi, a.x, a.y);
-  if (has_b) {
-    cmadd<(Y + 16) * RHO, N>(lr, li, b.x, b.y);
-    cmadd<(Y + 16) * (RHO + Q), N>(hr, hi, b.x, b.y);
-  }
-  z[bitrev4(Y)].re = make_float2(lr, hr);
-  z[bitrev4(Y)].im = make_float2(li, hi);
-}
-template <int Q, int RHO, int Y>
-__device__ __forceinline__ void fold_all(C2 (&z)[16], const float2* __restrict__ in, int stride, int n_valid) {
+// fold + ramp: z[bitrev(y)] = (in[y] + c in[y+16]) tw[y], y = 0..15, where tw[y] = W_N^{y rho} and
+// c = tw[16] = W_N^{16 rho} (so that c tw[y] is the ramp of element y + 16).  `in` strides by
+// `stride` float4 cells; elements y + 16 with y >= NB are structurally zero and are not read.
+// tw[y] is a float4 (wr, wr, wi, wi) at tw + y * tws; tw[0] = 1 is not read.
+template <int NB, int Y>
+__device__ __forceinline__ void fold_ramp(C2 (&z)[16], const float4* __restrict__ in, int stride,
+                                          const float4* __restrict__ tw, int tws, float2 cr, float2 ci) {
   if constexpr (Y < 16) {
-    const float2 zero = make_float2(0.0f, 0.0f);
-    const float2 a = (Y < n_valid) ? in[Y * stride] : zero;
-    const bool has_b = (Y + 16 < n_valid);
-    const float2 b = has_b ? in[(Y + 16) * stride] : zero;
-    fold_one<Q, RHO, Y>(z, a, b, has_b);
-    fold_all<Q, RHO, Y + 1>(z, in, stride, n_valid);
+    const float4 a = in[Y * stride];
+    float2 sr = make_float2(a.x, a.y), si = make_float2(a.z, a.w);
+    if constexpr (Y < NB) {
+      const float4 b = in[(Y + 16) * stride];
+      const float2 br = make_float2(b.x, b.y), bi = make_float2(b.z, b.w);
+      sr = __ffma2_rn(br, cr, sr); sr = __ffma2_rn(neg2(bi), ci, sr);
+      si = __ffma2_rn(bi, cr, si); si = __ffma2_rn(br, ci, si);
+    }
+    if constexpr (Y == 0) {
+      z[0].re = sr; z[0].im = si;
+    } else {
+      const float4 w = tw[Y * tws];
+      const float2 wr = make_float2(w.x, w.y), wi = make_float2(w.z, w.w);
+      const float2 t = __fmul2_rn(si, wi), u = __fmul2_rn(si, wr);
+      z[bitrev4(Y)].re = __ffma2_rn(sr, wr, neg2(t));
+      z[bitrev4(Y)].im = __ffma2_rn(sr, wi, u);
+    }
+    // bar.warp.sync is the one fence ptxas will not move shared loads across: without it all 32+15
+    // loads are hoisted to the top of the task and the accumulators spill (128-register budget)
+    if constexpr ((Y & (CHUNK - 1)) == CHUNK - 1 && Y < 15) __syncwarp();
+    fold_ramp<NB, Y + 1>(z, in, stride, tw, tws, cr, ci);
   }
-}
-
-// The 32-point pruned transform of this file's header: in[y], y < n_valid (<= 32), zero beyond.
-// z[k].lo = X[2Q k + RHO], z[k].hi = X[2Q k + RHO + Q].
-template <int Q, int RHO>
-__device__ __forceinline__ void dft32_pair(C2 (&z)[16], const float2* __restrict__ in, int stride, int n_valid) {
-  fold_all<Q, RHO, 0>(z, in, stride, n_valid);
-  fft16(z);
 }
 
 // ---------------------------------------------------------------- kernel parameters
@@ -190,165 +169,165 @@ struct FusedParams {
   const uint32_t* cell_info; // [32*32] dense block cells: (first entry << 8) | entry count
   const uint16_t* ent_ant;   // gather entries, sorted by block cell
   const float2* ent_tap;
-  int n_t, n_chan, n_ant, n_planes;
+  const float4* tw;          // [17][2Q]: (wr, wr, wi, wi) of exp(+2 pi i y rho / N), y = 0..16
+  int n_t, n_chan, n_ant, n_pol, n_planes;
   int R, Cc;                 // occupied rows / columns of the block
-  int nb;                    // batches per unit = ceil(n_t / Q)
+  int nb;                    // batches per unit
   long long total;           // n_chan * Q * nb batches in all
-  int row_bytes;             // NPOL * A
-  int row_pitch;             // row_bytes rounded up to 16
-  int aligned16;             // voltages can be staged with 16-byte cp.async
 };
 
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
-
-// S1 (reading Q1): byte hhhhllll -> ((h ^ 8) << 16) | (l ^ 8), i.e. both
-// two's-complement nibbles biased by +8 in the halves of one word, so a cell's samples can be
-// summed with one integer add.
-__device__ __forceinline__ uint32_t unpack_biased(uint32_t byte) {
-  return ((byte * 0x1001u) & 0x000F000Fu) ^ 0x00080008u;
-}
-__device__ __forceinline__ float small_int_to_float(int v) {  // exact for |v| < 2^22, no I2F
-  return __int_as_float(0x4B400000 + v) - 12582912.0f;
+// S1 (reading Q1).  Four samples per 32-bit word: high nibbles are the real
+// parts, low nibbles the imaginary parts, two's complement.  n ^ 8 = sext4(n) + 8 in 0..15;
+// dropping that byte into the mantissa of 12582912.0f (0x4B400000) and subtracting 12582920.0f
+// gives sext4(n) exactly, with no integer-to-float conversion instruction.
+__device__ __forceinline__ float biased_byte_to_float_bits(uint32_t w, int i) {
+  return __uint_as_float(__byte_perm(w, 0x4B400000u, 0x7650u + (uint32_t)i));
 }
 
-// stage the voltages of batch g (Q frames of one channel) into vs[FB][row_pitch]
-template <int Q, int NT>
-__device__ __forceinline__ void stage_voltages(const FusedParams& P, uint8_t* vs, int c, int b, int tid) {
-  const size_t frame_stride = (size_t)P.n_chan * P.row_bytes;
-  const uint8_t* src0 = P.volt + (size_t)c * P.row_bytes;
-  if (P.aligned16) {
-    const int chunks = P.row_pitch >> 4;
-    for (int i = tid; i < Q * chunks; i += NT) {
-      const int f = i / chunks, k = i - f * chunks;
-      const int t = b * Q + f;
-      uint8_t* dst = vs + f * P.row_pitch + k * 16;
-      if (t < P.n_t) cp_async16(dst, src0 + (size_t)t * frame_stride + k * 16);
-      else *reinterpret_cast<uint4*>(dst) = make_uint4(0u, 0u, 0u, 0u);
-    }
-  } else {
-    for (int i = tid; i < Q * P.row_bytes; i += NT) {
-      const int f = i / P.row_bytes, k = i - f * P.row_bytes;
-      const int t = b * Q + f;
-      vs[f * P.row_pitch + k] = (t < P.n_t) ? src0[(size_t)t * frame_stride + k] : (uint8_t)0;
+// word pair (lo plane, hi plane) of antennas a0..a0+3 -> E[a0..a0+3] = (re_lo, re_hi, im_lo, im_hi)
+__device__ __forceinline__ void unpack_words(uint32_t wlo, uint32_t whi, float4* __restrict__ e) {
+  const uint32_t rl = ((wlo >> 4) & 0x0F0F0F0Fu) ^ 0x08080808u, il = (wlo & 0x0F0F0F0Fu) ^ 0x08080808u;
+  const uint32_t rh = ((whi >> 4) & 0x0F0F0F0Fu) ^ 0x08080808u, ih = (whi & 0x0F0F0F0Fu) ^ 0x08080808u;
+  const float2 bias = f2(-12582920.0f);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const float2 re = __fadd2_rn(make_float2(biased_byte_to_float_bits(rl, i), biased_byte_to_float_bits(rh, i)), bias);
+    const float2 im = __fadd2_rn(make_float2(biased_byte_to_float_bits(il, i), biased_byte_to_float_bits(ih, i)), bias);
+    e[i] = make_float4(re.x, re.y, im.x, im.y);
+  }
+}
+
+// Per-thread voltage slots, fixed for the kernel's lifetime: slot k covers antennas a..a+3 of pair j
+// of every batch (j < 0: unused).  Voltage rows are read as aligned 32-bit words.
+struct PrefetchSlots {
+  int j[MAXW], a[MAXW];
+};
+
+template <int NT>
+__device__ __forceinline__ void prefetch_init(const FusedParams& P, int tid, PrefetchSlots& ps) {
+  const int ag = P.n_ant >> 2;
+#pragma unroll
+  for (int k = 0; k < MAXW; ++k) {
+    const int i = tid + k * NT;
+    ps.j[k] = -1; ps.a[k] = 0;
+    if (i < F * ag) { ps.j[k] = i / ag; ps.a[k] = (i - ps.j[k] * ag) << 2; }
+  }
+}
+
+// global -> registers: the voltages of batch b of channel c (F pairs x A antennas).  Time samples
+// past n_t read as the zero sample.
+template <int NT>
+__device__ __forceinline__ void prefetch_batch(const FusedParams& P, const PrefetchSlots& ps, int c, int b,
+                                               uint32_t (&wlo)[MAXW], uint32_t (&whi)[MAXW]) {
+  const int tmul = P.n_pol == 2 ? 1 : 2, thi = P.n_pol == 2 ? 0 : 1, hi_off = P.n_pol == 2 ? P.n_ant : 0;
+  const size_t row_bytes = (size_t)P.n_pol * P.n_ant;
+#pragma unroll
+  for (int k = 0; k < MAXW; ++k) {
+    wlo[k] = 0u; whi[k] = 0u;
+    if (ps.j[k] >= 0) {
+      const int t_lo = (b * F + ps.j[k]) * tmul, t_hi = t_lo + thi;
+      const uint8_t* base = P.volt + (size_t)c * row_bytes + ps.a[k];
+      if (t_lo < P.n_t) wlo[k] = __ldg(reinterpret_cast<const uint32_t*>(base + (size_t)t_lo * P.n_chan * row_bytes));
+      if (t_hi < P.n_t) whi[k] = __ldg(reinterpret_cast<const uint32_t*>(base + (size_t)t_hi * P.n_chan * row_bytes + hi_off));
     }
   }
-  cp_async_commit();
 }
 
-// S1 + S3 for the batch: every thread owns the block cells tid + j*NT and sums their gather
-// lists, in table order, for all Q*NPOL (frame, pol) planes.  A zero byte is the zero sample.
-template <int Q, int NPOL, int NT, bool DELTA>
-__device__ __forceinline__ void gather_batch(const FusedParams& P, const uint8_t* __restrict__ vs,
-                                             float2* __restrict__ gh, const uint32_t (&info)[S * S / NT],
-                                             int tid) {
-  constexpr int PL = Q * NPOL;
+// registers -> E[F][A] (float4 per antenna), S1
+__device__ __forceinline__ void unpack_batch(const FusedParams& P, const PrefetchSlots& ps, float4* __restrict__ E,
+                                             const uint32_t (&wlo)[MAXW], const uint32_t (&whi)[MAXW]) {
+#pragma unroll
+  for (int k = 0; k < MAXW; ++k)
+    if (ps.j[k] >= 0) unpack_words(wlo[k], whi[k], E + ps.j[k] * P.n_ant + ps.a[k]);
+}
+
+// S3 for the batch: every thread owns the block cells tid + j*NT and sums their gather lists,
+// in table order, for all F pair-planes (collisions sum).
+template <int NT, bool DELTA>
+__device__ __forceinline__ void gather_batch(const FusedParams& P, const float4* __restrict__ E,
+                                             float4* __restrict__ gh, const uint32_t (&info)[S * S / NT], int tid) {
 #pragma unroll
   for (int j = 0; j < S * S / NT; ++j) {
     const int cell = tid + j * NT;
     const int cy = cell >> 5, cx = cell & 31;
     if (cy >= P.R) continue;
     const uint32_t beg = info[j] >> 8, cnt = info[j] & 0xFFu;
-    float2* dst = gh + cy * HS + cx;
-    if (DELTA) {
-      uint32_t s[PL];
+    float2 sr[F], si[F];
 #pragma unroll
-      for (int pl = 0; pl < PL; ++pl) s[pl] = 0u;
-      for (uint32_t e = beg; e < beg + cnt; ++e) {
-        const int a = __ldg(P.ent_ant + e);
+    for (int f = 0; f < F; ++f) { sr[f] = make_float2(0.0f, 0.0f); si[f] = make_float2(0.0f, 0.0f); }
+    for (uint32_t e = beg; e < beg + cnt; ++e) {
+      const float4* ea = E + __ldg(P.ent_ant + e);
+      if (DELTA) {
 #pragma unroll
-        for (int pl = 0; pl < PL; ++pl) {
-          const int f = pl / NPOL, pol = pl % NPOL;
-          s[pl] += unpack_biased(vs[f * P.row_pitch + pol * P.n_ant + a]);
+        for (int f = 0; f < F; ++f) {
+          const float4 v = ea[f * P.n_ant];
+          sr[f] = __fadd2_rn(sr[f], make_float2(v.x, v.y));
+          si[f] = __fadd2_rn(si[f], make_float2(v.z, v.w));
         }
-      }
-      const int bias = 8 * (int)cnt;
-#pragma unroll
-      for (int pl = 0; pl < PL; ++pl) {
-        const float re = small_int_to_float((int)(s[pl] >> 16) - bias);
-        const float im = small_int_to_float((int)(s[pl] & 0xFFFFu) - bias);
-        dst[pl * (S * HS)] = make_float2(re, im);
-      }
-    } else {
-      float2 s[PL];
-#pragma unroll
-      for (int pl = 0; pl < PL; ++pl) s[pl] = make_float2(0.0f, 0.0f);
-      for (uint32_t e = beg; e < beg + cnt; ++e) {
-        const int a = __ldg(P.ent_ant + e);
+      } else {
         const float2 w = __ldg(P.ent_tap + e);
+        const float2 wr = f2(w.x), wi = f2(w.y);
 #pragma unroll
-        for (int pl = 0; pl < PL; ++pl) {
-          const int f = pl / NPOL, pol = pl % NPOL;
-          const uint32_t u = unpack_biased(vs[f * P.row_pitch + pol * P.n_ant + a]);
-          const float er = small_int_to_float((int)(u >> 16) - 8);
-          const float ei = small_int_to_float((int)(u & 0xFFFFu) - 8);
-          s[pl].x = fmaf(w.x, er, s[pl].x); s[pl].x = fmaf(-w.y, ei, s[pl].x);
-          s[pl].y = fmaf(w.x, ei, s[pl].y); s[pl].y = fmaf(w.y, er, s[pl].y);
+        for (int f = 0; f < F; ++f) {
+          const float4 v = ea[f * P.n_ant];
+          const float2 vr = make_float2(v.x, v.y), vi = make_float2(v.z, v.w);
+          sr[f] = __ffma2_rn(vr, wr, sr[f]); sr[f] = __ffma2_rn(neg2(vi), wi, sr[f]);
+          si[f] = __ffma2_rn(vi, wr, si[f]); si[f] = __ffma2_rn(vr, wi, si[f]);
         }
       }
-#pragma unroll
-      for (int pl = 0; pl < PL; ++pl) dst[pl * (S * HS)] = s[pl];
     }
+    float4* dst = gh + cy * HS + cx;
+#pragma unroll
+    for (int f = 0; f < F; ++f) dst[f * PLANE] = make_float4(sr[f].x, sr[f].y, si[f].x, si[f].y);
   }
 }
 
-// rows: thread = (frame f, pol, row y); in place on its own row of gh[f][pol]
-template <int Q, int RHO>
-__device__ __forceinline__ void row_task(float2* __restrict__ row, int n_valid) {
+// ---------------------------------------------------------------- the two transform roles
+// rows: thread = (pair f, row y, h); 32 cells of the row -> outputs l1 = 2k + h, in place.
+// The caller guarantees both h-threads of a row sit in one warp and separates loads from stores
+// with __syncwarp().
+template <int NB>
+__device__ __forceinline__ void row_task(float4* __restrict__ row, const float4* __restrict__ tw, int tws,
+                                         int h, bool valid) {
   C2 z[16];
-  dft32_pair<Q, RHO>(z, row, 1, n_valid);
-  // output k: lo -> l1 = 2k, hi -> l1 = 2k+1 (l = Q l1 + l2): one 16-byte store per k
-  float4* out = reinterpret_cast<float4*>(row);
+  const float4 c = tw[16 * tws];
+  fold_ramp<NB, 0>(z, row, 1, tw, tws, make_float2(c.x, c.y), make_float2(c.z, c.w));
+  fft16(z);
+  __syncwarp();
+  if (valid) {
 #pragma unroll
-  for (int k = 0; k < 16; ++k) out[k] = make_float4(z[k].re.x, z[k].im.x, z[k].re.y, z[k].im.y);
+    for (int k = 0; k < 16; ++k) row[2 * k + h] = make_float4(z[k].re.x, z[k].re.y, z[k].im.x, z[k].im.y);
+  }
 }
 
-// columns + S5 + S6: thread = (pol, m2 = RHO, l1); acc[k] = (m = 2Q k + RHO, m = 2Q k + RHO + Q)
-template <int Q, int RHO>
-__device__ __forceinline__ void col_task_power(const float2* __restrict__ col, int n_valid, float2 (&acc)[16]) {
+// columns + S5 + S6: thread = (l1, rho); outputs m = 2Q k + rho, k = 0..15.
+// acc[k] = (|A_lo|^2, |A_hi|^2) sums; xy[k] = sum of A_lo conj(A_hi) (reading Q11) when NPROD == 4.
+template <int NB, int NPROD>
+__device__ __forceinline__ void col_task(const float4* __restrict__ col, const float4* __restrict__ tw, int tws,
+                                         float2 cr, float2 ci, float2 (&acc)[16],
+                                         float2 (&xy)[NPROD == 4 ? 16 : 1]) {
   C2 z[16];
-  dft32_pair<Q, RHO>(z, col, HS, n_valid);
+  fold_ramp<NB, 0>(z, col, HS, tw, tws, cr, ci);
+  fft16(z);
 #pragma unroll
   for (int k = 0; k < 16; ++k) {
     acc[k] = __ffma2_rn(z[k].re, z[k].re, acc[k]);
     acc[k] = __ffma2_rn(z[k].im, z[k].im, acc[k]);
+    if constexpr (NPROD == 4) {
+      xy[k].x = fmaf(z[k].re.x, z[k].re.y, xy[k].x); xy[k].x = fmaf(z[k].im.x, z[k].im.y, xy[k].x);
+      xy[k].y = fmaf(z[k].im.x, z[k].re.y, xy[k].y); xy[k].y = fmaf(-z[k].re.x, z[k].im.y, xy[k].y);
+    }
   }
 }
 
-template <int Q, int R0>
-__device__ __forceinline__ void row_dispatch(int rho, float2* row, int n_valid) {
-  if constexpr (R0 < Q) {
-    if (rho == R0) row_task<Q, R0>(row, n_valid);
-    else row_dispatch<Q, R0 + 1>(rho, row, n_valid);
-  }
-}
-template <int Q, int R0>
-__device__ __forceinline__ void col_dispatch(int rho, const float2* col, int n_valid, float2 (&acc)[16]) {
-  if constexpr (R0 < Q) {
-    if (rho == R0) col_task_power<Q, R0>(col, n_valid, acc);
-    else col_dispatch<Q, R0 + 1>(rho, col, n_valid, acc);
-  }
-}
-
-template <int Q, int NPOL>
-struct FusedGeo {
-  static constexpr int NT = NPOL * Q * 32;                 // threads per CTA
-  static constexpr int PLANE = S * HS;                     // complex elements per (frame, pol) plane
-  static constexpr size_t GH_BYTES = (size_t)Q * NPOL * PLANE * sizeof(float2);
-};
-
-template <int Q, int NPOL, bool DELTA>
-__global__ void __launch_bounds__(NPOL * Q * 32, (NPOL * Q * 32 <= 256) ? 2 : 1)
+template <int Q, int NPROD, bool DELTA, int NB>
+__global__ void __launch_bounds__(64 * Q, NPROD == 4 ? 1 : 2)
 epic_fused_kernel(FusedParams P) {
-  using G = FusedGeo<Q, NPOL>;
-  constexpr int NT = G::NT, N = 32 * Q;
+  constexpr int NT = 64 * Q, N = 32 * Q, TWS = 2 * Q;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  float2* gh = reinterpret_cast<float2*>(smem_raw);        // [Q][NPOL][32][HS]
-  uint8_t* vs = smem_raw + G::GH_BYTES;                    // [2][Q][row_pitch]
+  float4* gh = reinterpret_cast<float4*>(smem_raw);  // [F][32][HS]
+  float4* tws = gh + F * PLANE;                      // [17][2Q]
+  float4* E = tws + 17 * TWS;                        // [F][A]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
   // static, contiguous share of the (unit-major, batch-minor) work list
@@ -359,80 +338,139 @@ epic_fused_kernel(FusedParams P) {
   uint32_t info[S * S / NT];
 #pragma unroll
   for (int j = 0; j < S * S / NT; ++j) info[j] = __ldg(P.cell_info + tid + j * NT);
+  for (int i = tid; i < F * PLANE; i += NT) gh[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);  // rows >= R stay zero
+  for (int i = tid; i < 17 * TWS; i += NT) tws[i] = __ldg(P.tw + i);
+  __syncthreads();
 
-  // column-stage role: warp -> m2, lanes -> (pol, l1)
-  const int m2 = warp / NPOL;
-  const int pol_c = (NPOL == 2) ? (lane >> 4) : 0;
-  const int l1 = (NPOL == 2) ? ((warp & 1) * 16 + (lane & 15)) : lane;
-  // row-stage role: warp -> (frame, pol), lane -> row
-  const int f_r = warp / NPOL, pol_r = warp % NPOL;
+  // column role: 8 consecutive l1 x 4 residues per warp (a warp reads 128 contiguous bytes per row)
+  const int l1 = (warp & 3) * 8 + (lane & 7);
+  const int rho = (warp >> 2) * 4 + (lane >> 3);
+  const float4 c_col = tws[16 * TWS + rho];
+  const float2 cr_c = make_float2(c_col.x, c_col.y), ci_c = make_float2(c_col.z, c_col.w);
 
   float2 acc[16];
+  float2 xy[NPROD == 4 ? 16 : 1];
 #pragma unroll
   for (int k = 0; k < 16; ++k) acc[k] = make_float2(0.0f, 0.0f);
+#pragma unroll
+  for (int k = 0; k < (NPROD == 4 ? 16 : 1); ++k) xy[k] = make_float2(0.0f, 0.0f);
 
   auto flush = [&](int unit) {
     const int c = unit / Q, l2 = unit - c * Q;
-    float* o = P.out + ((size_t)c * P.n_planes + pol_c) * (size_t)(N * N) + (Q * l1 + l2);
+    const size_t plane = (size_t)N * N;
+    float* o = P.out + (size_t)c * P.n_planes * plane + (Q * l1 + l2);
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
-      atomicAdd(o + (size_t)(2 * Q * k + m2) * N, acc[k].x);
-      atomicAdd(o + (size_t)(2 * Q * k + m2 + Q) * N, acc[k].y);
+      float* px = o + (size_t)(2 * Q * k + rho) * N;
+      if constexpr (NPROD == 1) {
+        atomicAdd(px, acc[k].x + acc[k].y);
+      } else {
+        atomicAdd(px, acc[k].x);
+        atomicAdd(px + plane, acc[k].y);
+      }
+      if constexpr (NPROD == 4) {  // YX = conj(XY)
+        atomicAdd(px + 2 * plane, xy[k].x);
+        atomicAdd(px + 3 * plane, xy[k].y);
+        atomicAdd(px + 4 * plane, xy[k].x);
+        atomicAdd(px + 5 * plane, -xy[k].y);
+        xy[k] = make_float2(0.0f, 0.0f);
+      }
       acc[k] = make_float2(0.0f, 0.0f);
     }
   };
 
   int unit = (int)(g0 / P.nb);
   int b = (int)(g0 - (long long)unit * P.nb);
-  int buf = 0;
-  stage_voltages<Q, NT>(P, vs, unit / Q, b, tid);
+  PrefetchSlots ps;
+  prefetch_init<NT>(P, tid, ps);
+  uint32_t wlo[MAXW], whi[MAXW];
+  prefetch_batch<NT>(P, ps, unit / Q, b, wlo, whi);
+  unpack_batch(P, ps, E, wlo, whi);
+  __syncthreads();
+
+  const int ntask = F * P.R * 2;
   for (long long g = g0; g < g1; ++g) {
-    cp_async_wait_all();
-    __syncthreads();  // this batch's voltages are visible; previous column stage is done with gh
-    // prefetch the next batch
     int unit_n = unit, b_n = b + 1;
     if (b_n == P.nb) { b_n = 0; ++unit_n; }
-    if (g + 1 < g1) stage_voltages<Q, NT>(P, vs + (buf ^ 1) * Q * P.row_pitch, unit_n / Q, b_n, tid);
+    const bool more = g + 1 < g1;
+    if (more) prefetch_batch<NT>(P, ps, unit_n / Q, b_n, wlo, whi);
 
-    gather_batch<Q, NPOL, NT, DELTA>(P, vs + buf * Q * P.row_pitch, gh, info, tid);
+    gather_batch<NT, DELTA>(P, E, gh, info, tid);
     __syncthreads();
-    if (lane < P.R) row_dispatch<Q, 0>(unit % Q, gh + (f_r * NPOL + pol_r) * G::PLANE + lane * HS, P.Cc);
+
+    const int l2 = unit % Q;
+    for (int base = warp * 32; base < ntask; base += NT) {
+      const int task = base + lane;
+      const bool valid = task < ntask;
+      // idle lanes transform the all-zero row 31 of plane 0 (never written: they exist only when R < 32)
+      int f = 0, y = S - 1, h = 0;
+      if (valid) { h = task & 1; const int p = task >> 1; f = p / P.R; y = p - f * P.R; }
+      row_task<NB>(gh + f * PLANE + y * HS, tws + (l2 + Q * h), TWS, h, valid);
+    }
     __syncthreads();
+
+    if (more) unpack_batch(P, ps, E, wlo, whi);  // E was last read by this batch's gather
 #pragma unroll 1
-    for (int f = 0; f < Q; ++f)
-      col_dispatch<Q, 0>(m2, gh + (f * NPOL + pol_c) * G::PLANE + l1, P.R, acc);
+    for (int f = 0; f < F; ++f) {
+      // launder the table pointer: the 15 twiddles must be re-read per task, not held in 60 registers
+      int tw_off = rho;
+      asm volatile("" : "+r"(tw_off));
+      col_task<NB, NPROD>(gh + f * PLANE + l1, tws + tw_off, TWS, cr_c, ci_c, acc, xy);
+    }
 
-    if (unit_n != unit || g + 1 == g1) flush(unit);
-    unit = unit_n; b = b_n; buf ^= 1;
+    if (unit_n != unit || !more) flush(unit);
+    unit = unit_n; b = b_n;
+    __syncthreads();  // next batch's E is complete; gh is free
   }
 }
 
 struct FusedTables {
   uint32_t* cell_info;
+  float4* tw;
 };
 
-template <int Q, int NPOL, bool DELTA>
+template <int Q>
+size_t fused_smem_bytes(int n_ant) {
+  return ((size_t)F * PLANE + (size_t)17 * 2 * Q + (size_t)F * n_ant) * sizeof(float4);
+}
+
+template <int Q, int NPROD, bool DELTA, int NB>
 int launch_fused(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
-  using G = FusedGeo<Q, NPOL>;
-  const size_t smem = G::GH_BYTES + (size_t)2 * Q * P.row_pitch;
-  auto kern = epic_fused_kernel<Q, NPOL, DELTA>;
+  constexpr int NT = 64 * Q;
+  const size_t smem = fused_smem_bytes<Q>(P.n_ant);
+  auto kern = epic_fused_kernel<Q, NPROD, DELTA, NB>;
   if (smem > 48 * 1024)
     EPIC_CUDA_TRY(cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int per_sm = 0;
-  EPIC_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, G::NT, smem));
+  EPIC_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NT, smem));
   if (per_sm < 1) return EPIC_ERR_RANGE;
   const long long slots = (long long)per_sm * p->n_sm;
   const int grid = (int)std::min<long long>(P.total, slots);
-  kern<<<grid, G::NT, smem, s>>>(P);
+  kern<<<grid, NT, smem, s>>>(P);
   EPIC_CUDA_TRY(cudaGetLastError());
   return EPIC_OK;
 }
 
+template <int Q, int NPROD, bool DELTA>
+int launch_fused_nb(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
+  // elements y + 16 of a row/column are read only while y < NB (the rest of the block is empty)
+  if (std::max(p->R, p->Cc) <= 16 + 12) return launch_fused<Q, NPROD, DELTA, 12>(p, P, s);
+  return launch_fused<Q, NPROD, DELTA, 16>(p, P, s);
+}
+
 template <int Q>
-int launch_fused_q(const epic_plan* p, const FusedParams& P, int n_pol, cudaStream_t s) {
+int launch_fused_q(const epic_plan* p, const FusedParams& P, int n_products, cudaStream_t s) {
   const bool delta = p->t.is_delta != 0;
-  if (n_pol == 1) return delta ? launch_fused<Q, 1, true>(p, P, s) : launch_fused<Q, 1, false>(p, P, s);
-  return delta ? launch_fused<Q, 2, true>(p, P, s) : launch_fused<Q, 2, false>(p, P, s);
+#ifdef EPIC_FUSED_DEV_ONE  // development builds: compile a single instantiation
+  if (Q == 4 && n_products == 2 && delta) return launch_fused<4, 2, true, 12>(p, P, s);
+  return EPIC_ERR_RANGE;
+#else
+  switch (n_products) {
+    case 1: return delta ? launch_fused_nb<Q, 1, true>(p, P, s) : launch_fused_nb<Q, 1, false>(p, P, s);
+    case 2: return delta ? launch_fused_nb<Q, 2, true>(p, P, s) : launch_fused_nb<Q, 2, false>(p, P, s);
+    default: return delta ? launch_fused_nb<Q, 4, true>(p, P, s) : launch_fused_nb<Q, 4, false>(p, P, s);
+  }
+#endif
 }
 
 }  // namespace
@@ -450,15 +488,28 @@ int fused_plan_init(epic_plan* p) {
     if (c.ent_count > 255u) return EPIC_OK;  // falls back to the two-pass path
     info[(size_t)c.y * S + c.x] = (c.ent_begin << 8) | c.ent_count;
   }
+  // ramp table exp(+2 pi i y rho / N), y = 0..16, rho = 0..2Q-1, from double (reading Q8: + sign)
+  std::vector<float4> tw((size_t)17 * 2 * Q);
+  for (int y = 0; y <= 16; ++y)
+    for (int rho = 0; rho < 2 * Q; ++rho) {
+      const int ex = (y * rho) % p->N;
+      const double ang = 2.0 * M_PI * (double)ex / (double)p->N;
+      const float wr = (float)std::cos(ang), wi = (float)std::sin(ang);
+      tw[(size_t)y * 2 * Q + rho] = make_float4(wr, wr, wi, wi);
+    }
   FusedTables* ft = new (std::nothrow) FusedTables();
   if (!ft) return EPIC_ERR_NOMEM;
   ft->cell_info = nullptr;
+  ft->tw = nullptr;
   cudaError_t ce = cudaMalloc(&ft->cell_info, info.size() * sizeof(uint32_t));
+  if (ce == cudaSuccess) ce = cudaMalloc(&ft->tw, tw.size() * sizeof(float4));
   if (ce == cudaSuccess)
     ce = cudaMemcpy(ft->cell_info, info.data(), info.size() * sizeof(uint32_t), cudaMemcpyHostToDevice);
+  if (ce == cudaSuccess) ce = cudaMemcpy(ft->tw, tw.data(), tw.size() * sizeof(float4), cudaMemcpyHostToDevice);
   if (ce != cudaSuccess) {
     set_cuda_error(ce);
     if (ft->cell_info) cudaFree(ft->cell_info);
+    if (ft->tw) cudaFree(ft->tw);
     delete ft;
     return ce == cudaErrorMemoryAllocation ? EPIC_ERR_NOMEM : EPIC_ERR_CUDA;
   }
@@ -471,6 +522,7 @@ void fused_plan_free(epic_plan* p) {
   FusedTables* ft = static_cast<FusedTables*>(p->d_fused);
   if (ft) {
     if (ft->cell_info) cudaFree(ft->cell_info);
+    if (ft->tw) cudaFree(ft->tw);
     delete ft;
   }
   p->d_fused = nullptr;
@@ -479,10 +531,12 @@ void fused_plan_free(epic_plan* p) {
 
 int fused_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products) {
   if (!p->fused_ok || is_cf32) return 0;
-  if (n_products != n_pol) return 0;  // {XX} or {XX, YY}
-  const size_t pitch = ((size_t)n_pol * p->n_ant + 15) & ~(size_t)15;
+  if (!((n_pol == 1 && n_products == 1) || (n_pol == 2 && (n_products == 2 || n_products == 4)))) return 0;
   const int Q = p->N / S;
-  const size_t smem = (size_t)Q * n_pol * S * HS * sizeof(float2) + 2 * Q * pitch;
+  const int nt = 64 * Q;
+  if (p->n_ant % 4 != 0) return 0;  // voltage rows are read as 32-bit words
+  if ((long long)F * (p->n_ant / 4) > (long long)MAXW * nt) return 0;  // prefetch registers
+  const size_t smem = Q == 2 ? fused_smem_bytes<2>(p->n_ant) : fused_smem_bytes<4>(p->n_ant);
   return smem <= (size_t)200 * 1024 ? 1 : 0;
 }
 
@@ -495,20 +549,20 @@ int fused_image(epic_plan* p, const ImageArgs& a) {
   P.cell_info = ft->cell_info;
   P.ent_ant = p->t.ent_ant;
   P.ent_tap = p->t.ent_tap;
+  P.tw = ft->tw;
   P.n_t = a.n_t;
   P.n_chan = a.n_chan;
   P.n_ant = p->n_ant;
+  P.n_pol = a.n_pol;
   P.n_planes = a.n_planes;
   P.R = p->R;
   P.Cc = p->Cc;
-  P.nb = (a.n_t + Q - 1) / Q;
+  const int per_batch = a.n_pol == 2 ? F : 2 * F;  // time samples per batch
+  P.nb = (a.n_t + per_batch - 1) / per_batch;
   P.total = (long long)a.n_chan * Q * P.nb;
-  P.row_bytes = a.n_pol * p->n_ant;
-  P.row_pitch = (P.row_bytes + 15) & ~15;
-  P.aligned16 = (P.row_bytes % 16 == 0 && (reinterpret_cast<uintptr_t>(a.volt) & 15u) == 0) ? 1 : 0;
   int st;
-  if (Q == 2) st = launch_fused_q<2>(p, P, a.n_pol, a.stream);
-  else st = launch_fused_q<4>(p, P, a.n_pol, a.stream);
+  if (Q == 2) st = launch_fused_q<2>(p, P, a.n_products, a.stream);
+  else st = launch_fused_q<4>(p, P, a.n_products, a.stream);
   if (st != EPIC_OK) return st;
   p->last_launches = 1;
   return EPIC_OK;

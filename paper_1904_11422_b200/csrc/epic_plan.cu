@@ -188,7 +188,9 @@ static int image_common(epic_plan* plan, const void* volt, int is_cf32, int n_t,
   a.out = out;
   a.stream = (cudaStream_t)stream;
   int path = plan->path_req;
-  const int fused_can = fused_supported(plan, is_cf32, n_pol, n_products);
+  // the fused kernel reads voltage rows as 32-bit words
+  const int fused_can = fused_supported(plan, is_cf32, n_pol, n_products) &&
+                        (reinterpret_cast<uintptr_t>(volt) & 3u) == 0;
   if (path == EPIC_PATH_AUTO) path = fused_can ? EPIC_PATH_FUSED : EPIC_PATH_TWOPASS;
   if (path == EPIC_PATH_FUSED) {
     if (!fused_can) return EPIC_ERR_RANGE;
