@@ -51,6 +51,24 @@ def algorithmic_bytes_per_frame(wl) -> float:
     return v + img
 
 
+def max_over_ranks(values, device) -> list:
+    """Element-wise MAX of a list of floats over all ranks (identity for a single process)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return [float(v) for v in values]
+    tt = torch.tensor(list(values), dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return [float(v) for v in tt.cpu()]
+
+
+def channel_shard(n_chan: int, rank: int, world: int):
+    """Channels [lo, hi) of rank `rank` when ONE workload is split over ranks (channels are
+    independent: no collective).  bench.py itself runs weak scaling (one full
+    workload per GPU); this is the strong-scaling split a deployment would use."""
+    return (n_chan * rank) // world, (n_chan * (rank + 1)) // world
+
+
 class ClockSampler:
     QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -64,7 +82,7 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.QUERY}",
-                 "--format=csv,noheader,nounits", "-lms", "100"],
+                 "--format=csv,noheader,nounits", "-lms", "20"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except OSError:
             self.proc = None
@@ -202,7 +220,6 @@ def run_epic(args, wl):
         sampler.start()
     evs = [step_device() for _ in range(args.steps)]
     barrier()
-    clocks = sampler.stop() if rank == 0 else None
     launches = plan.last_launches() * args.steps
     dev_ms = [a.elapsed_time(b) for a, b in evs]
     total_ms = float(sum(dev_ms))
@@ -212,12 +229,10 @@ def run_epic(args, wl):
     barrier()
     evs = [step_e2e() for _ in range(args.steps)]
     barrier()
+    clocks = sampler.stop() if rank == 0 else None  # sampled over both timed regions
     e2e_ms = float(sum(a.elapsed_time(b) for a, b in evs))
 
-    if world > 1:
-        tt = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms, e2e_ms = float(tt[0]), float(tt[1])
+    total_ms, e2e_ms = max_over_ranks([total_ms, e2e_ms], dev)
     path = plan.path(wl.n_pol)
     support = plan.support()
     probe = epic.epic_fp32_peak_probe(20000) if rank == 0 else None
@@ -274,7 +289,7 @@ def run_epic(args, wl):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (1-based)")
     ap.add_argument("--impl", default="epic", choices=["epic", "reference"])

@@ -49,117 +49,98 @@ constexpr int F = 4;         // pairs per batch
 constexpr int MAXW = 2;      // prefetched word pairs per thread
 constexpr int CHUNK = 2;     // fold_ramp: elements whose loads may be in flight together
 
-// ---------------------------------------------------------------- compile-time twiddles
-// exp(+2 pi i ex / n) in double, evaluated by the compiler (reading Q8: + sign, inverse DFT).
-constexpr double kPi = 3.14159265358979323846264338327950288;
-constexpr double sin_small(double x) {
-  const double x2 = x * x;
-  double term = x, sum = x;
-  for (int i = 1; i <= 12; ++i) { term *= -x2 / (double)((2 * i) * (2 * i + 1)); sum += term; }
-  return sum;
-}
-constexpr double cos_small(double x) {
-  const double x2 = x * x;
-  double term = 1.0, sum = 1.0;
-  for (int i = 1; i <= 12; ++i) { term *= -x2 / (double)((2 * i - 1) * (2 * i)); sum += term; }
-  return sum;
-}
-constexpr int mod_pos(int a, int n) { return ((a % n) + n) % n; }
-constexpr double tw_cos(int ex, int n) {
-  ex = mod_pos(ex, n);
-  const int j = (4 * ex + n / 2) / n;  // nearest quarter turn
-  const double phi = 2.0 * kPi * (double)(4 * ex - j * n) / (4.0 * (double)n);
-  const double cs = cos_small(phi), sn = sin_small(phi);
-  switch (j & 3) { case 0: return cs; case 1: return -sn; case 2: return -cs; default: return sn; }
-}
-constexpr double tw_sin(int ex, int n) {
-  ex = mod_pos(ex, n);
-  const int j = (4 * ex + n / 2) / n;
-  const double phi = 2.0 * kPi * (double)(4 * ex - j * n) / (4.0 * (double)n);
-  const double cs = cos_small(phi), sn = sin_small(phi);
-  switch (j & 3) { case 0: return sn; case 1: return cs; case 2: return -sn; default: return -cs; }
-}
-constexpr int bitrev4(int v) { return ((v & 1) << 3) | ((v & 2) << 1) | ((v & 4) >> 1) | ((v & 8) >> 3); }
+constexpr int TWV = 5;       // float4 words of twiddles per residue (TwSet)
 
 // ---------------------------------------------------------------- packed complex pair
 struct C2 { float2 re, im; };  // (lo, hi) halves = two independent planes
 
-__device__ __forceinline__ float2 f2(float v) { return make_float2(v, v); }
+__device__ __forceinline__ float2 f2(float v) { return make_float2(v, v); }  // FFMA2 takes it as one .F32 operand
 __device__ __forceinline__ float2 neg2(float2 v) { return make_float2(-v.x, -v.y); }
 
-// radix-2 DIT butterfly on packed pairs: (a, b) <- (a + w b, a - w b), w = exp(2 pi i K / NN)
-template <int K, int NN>
-__device__ __forceinline__ void bfly(C2& a, C2& b) {
-  if constexpr (K == 0) {
-    const C2 p = {__fadd2_rn(a.re, b.re), __fadd2_rn(a.im, b.im)};
-    b.re = __fadd2_rn(a.re, neg2(b.re)); b.im = __fadd2_rn(a.im, neg2(b.im));
-    a = p;
-  } else if constexpr (4 * K == NN) {  // w = +i: w b = (-b.im, b.re)
-    const C2 p = {__fadd2_rn(a.re, neg2(b.im)), __fadd2_rn(a.im, b.re)};
-    const C2 q = {__fadd2_rn(a.re, b.im), __fadd2_rn(a.im, neg2(b.re))};
-    a = p; b = q;
-  } else {
-    constexpr float wr = (float)tw_cos(K, NN), wi = (float)tw_sin(K, NN);
-    C2 p;
-    p.re = __ffma2_rn(b.re, f2(wr), a.re); p.re = __ffma2_rn(neg2(b.im), f2(wi), p.re);
-    p.im = __ffma2_rn(b.im, f2(wr), a.im); p.im = __ffma2_rn(b.re, f2(wi), p.im);
-    b.re = __ffma2_rn(a.re, f2(2.0f), neg2(p.re));
-    b.im = __ffma2_rn(a.im, f2(2.0f), neg2(p.im));
-    a = p;
-  }
+// The transform one thread computes (rows and columns alike):
+//
+//   X[k] = sum_{y<32} in[y] r^y W_16^{y k},  k = 0..15,   r = W_N^{rho}  (|r| = 1)
+//        = sum_{y<16} (in[y] + r^16 in[y+16]) r^y W_16^{y k}
+//
+// The residue ramp r^y is absorbed into the butterflies: decimation in time gives, for a length-n
+// sub-transform T_n(s, r_n),  T_n[k], T_n[k + n/2] = T_{n/2}(s_even, r_n^2)[k] +- (r_n W_n^k) T_{n/2}(s_odd, r_n^2)[k],
+// so level n = 2, 4, 8, 16 uses the twiddles r^{16/n} W_n^k: nine complex numbers per residue
+// (W_n^{k + n/4} = i W_n^k is a register swap), computed in double on the host.
+struct TwSet {
+  float cr, ci;              // r^16        (fold)
+  float w2r, w2i;            // r^8         (level 2)
+  float w4r, w4i;            // r^4         (level 4, k = 0; k = 1 is i times it)
+  float w8r[2], w8i[2];      // r^2 W_8^k   (level 8, k = 0, 1)
+  float w16r[4], w16i[4];    // r W_16^k    (level 16, k = 0..3)
+};
+
+// shared-memory image of a TwSet: TWV float4 words
+//   [0] = (cr, ci, w2r, w2i)  [1] = (w4r, w4i, w8r0, w8i0)  [2] = (w8r1, w8i1, w16r0, w16i0)
+//   [3] = (w16r1, w16i1, w16r2, w16i2)  [4] = (w16r3, w16i3, 0, 0)
+
+// radix-2 DIT butterfly on packed pairs: (a, b) <- (a + w b, a - w b); 6 FFMA2
+__device__ __forceinline__ void bfly(C2& a, C2& b, float wr, float wi) {
+  C2 p;
+  p.re = __ffma2_rn(b.re, f2(wr), a.re); p.re = __ffma2_rn(neg2(b.im), f2(wi), p.re);
+  p.im = __ffma2_rn(b.im, f2(wr), a.im); p.im = __ffma2_rn(b.re, f2(wi), p.im);
+  b.re = __ffma2_rn(a.re, f2(2.0f), neg2(p.re));
+  b.im = __ffma2_rn(a.im, f2(2.0f), neg2(p.im));
+  a = p;
 }
-template <int NN, int BASE, int K>
-__device__ __forceinline__ void fft16_block(C2 (&z)[16]) {
-  if constexpr (K < NN / 2) {
-    bfly<K, NN>(z[BASE + K], z[BASE + K + NN / 2]);
-    fft16_block<NN, BASE, K + 1>(z);
+// the same with twiddle i w = (-wi, wr)
+__device__ __forceinline__ void bfly_i(C2& a, C2& b, float wr, float wi) { bfly(a, b, -wi, wr); }
+
+// z holds s[y] = in[y] + r^16 in[y+16] in bit-reversed order; on return z[k] = X[k].
+// Twiddles are read from the residue's shared-memory TwSet level by level (short live ranges).
+__device__ __forceinline__ void fft16_ramped(C2 (&z)[16], const float4* __restrict__ tw, float w2r, float w2i) {
+#pragma unroll
+  for (int b = 0; b < 16; b += 2) bfly(z[b], z[b + 1], w2r, w2i);
+  const float4 t1 = tw[1];
+#pragma unroll
+  for (int b = 0; b < 16; b += 4) { bfly(z[b], z[b + 2], t1.x, t1.y); bfly_i(z[b + 1], z[b + 3], t1.x, t1.y); }
+  const float4 t2 = tw[2];
+#pragma unroll
+  for (int b = 0; b < 16; b += 8) {
+    bfly(z[b], z[b + 4], t1.z, t1.w);   bfly(z[b + 1], z[b + 5], t2.x, t2.y);
+    bfly_i(z[b + 2], z[b + 6], t1.z, t1.w); bfly_i(z[b + 3], z[b + 7], t2.x, t2.y);
   }
-}
-template <int NN, int BASE>
-__device__ __forceinline__ void fft16_stage(C2 (&z)[16]) {
-  if constexpr (BASE < 16) {
-    fft16_block<NN, BASE, 0>(z);
-    fft16_stage<NN, BASE + NN>(z);
-  }
-}
-// z holds the input in bit-reversed order; on return z[k] = sum_y in[y] exp(+2 pi i y k / 16).
-__device__ __forceinline__ void fft16(C2 (&z)[16]) {
-  fft16_stage<2, 0>(z);
-  fft16_stage<4, 0>(z);
-  fft16_stage<8, 0>(z);
-  fft16_stage<16, 0>(z);
+  const float4 t3 = tw[3], t4 = tw[4];
+  bfly(z[0], z[8], t2.z, t2.w);    bfly(z[1], z[9], t3.x, t3.y);
+  bfly(z[2], z[10], t3.z, t3.w);   bfly(z[3], z[11], t4.x, t4.y);
+  bfly_i(z[4], z[12], t2.z, t2.w); bfly_i(z[5], z[13], t3.x, t3.y);
+  bfly_i(z[6], z[14], t3.z, t3.w); bfly_i(z[7], z[15], t4.x, t4.y);
 }
 
-// fold + ramp: z[bitrev(y)] = (in[y] + c in[y+16]) tw[y], y = 0..15, where tw[y] = W_N^{y rho} and
-// c = tw[16] = W_N^{16 rho} (so that c tw[y] is the ramp of element y + 16).  `in` strides by
-// `stride` float4 cells; elements y + 16 with y >= NB are structurally zero and are not read.
-// tw[y] is a float4 (wr, wr, wi, wi) at tw + y * tws; tw[0] = 1 is not read.
+constexpr int bitrev4(int v) { return ((v & 1) << 3) | ((v & 2) << 1) | ((v & 4) >> 1) | ((v & 8) >> 3); }
+
+// fold: z[bitrev(y)] = in[y] + c in[y+16], y = 0..15, c = r^16.  `in` strides by `stride` float4
+// cells; elements y + 16 with y >= NB are structurally zero and are not read.
 template <int NB, int Y>
-__device__ __forceinline__ void fold_ramp(C2 (&z)[16], const float4* __restrict__ in, int stride,
-                                          const float4* __restrict__ tw, int tws, float2 cr, float2 ci) {
+__device__ __forceinline__ void fold(C2 (&z)[16], const float4* __restrict__ in, int stride, float cr, float ci) {
   if constexpr (Y < 16) {
     const float4 a = in[Y * stride];
     float2 sr = make_float2(a.x, a.y), si = make_float2(a.z, a.w);
     if constexpr (Y < NB) {
       const float4 b = in[(Y + 16) * stride];
       const float2 br = make_float2(b.x, b.y), bi = make_float2(b.z, b.w);
-      sr = __ffma2_rn(br, cr, sr); sr = __ffma2_rn(neg2(bi), ci, sr);
-      si = __ffma2_rn(bi, cr, si); si = __ffma2_rn(br, ci, si);
+      sr = __ffma2_rn(br, f2(cr), sr); sr = __ffma2_rn(neg2(bi), f2(ci), sr);
+      si = __ffma2_rn(bi, f2(cr), si); si = __ffma2_rn(br, f2(ci), si);
     }
-    if constexpr (Y == 0) {
-      z[0].re = sr; z[0].im = si;
-    } else {
-      const float4 w = tw[Y * tws];
-      const float2 wr = make_float2(w.x, w.y), wi = make_float2(w.z, w.w);
-      const float2 t = __fmul2_rn(si, wi), u = __fmul2_rn(si, wr);
-      z[bitrev4(Y)].re = __ffma2_rn(sr, wr, neg2(t));
-      z[bitrev4(Y)].im = __ffma2_rn(sr, wi, u);
-    }
-    // bar.warp.sync is the one fence ptxas will not move shared loads across: without it all 32+15
+    z[bitrev4(Y)].re = sr; z[bitrev4(Y)].im = si;
+    // bar.warp.sync is the one fence ptxas will not move shared loads across: without it all
     // loads are hoisted to the top of the task and the accumulators spill (128-register budget)
     if constexpr ((Y & (CHUNK - 1)) == CHUNK - 1 && Y < 15) __syncwarp();
-    fold_ramp<NB, Y + 1>(z, in, stride, tw, tws, cr, ci);
+    fold<NB, Y + 1>(z, in, stride, cr, ci);
   }
+}
+
+// One whole transform: `tw` points at the residue's TwSet words in shared memory.
+template <int NB>
+__device__ __forceinline__ void transform32(C2 (&z)[16], const float4* __restrict__ in, int stride,
+                                            const float4* __restrict__ tw) {
+  const float4 t0 = tw[0];
+  fold<NB, 0>(z, in, stride, t0.x, t0.y);
+  fft16_ramped(z, tw, t0.z, t0.w);
 }
 
 // ---------------------------------------------------------------- kernel parameters
@@ -169,7 +150,7 @@ struct FusedParams {
   const uint32_t* cell_info; // [32*32] dense block cells: (first entry << 8) | entry count
   const uint16_t* ent_ant;   // gather entries, sorted by block cell
   const float2* ent_tap;
-  const float4* tw;          // [17][2Q]: (wr, wr, wi, wi) of exp(+2 pi i y rho / N), y = 0..16
+  const float4* tw;          // [2Q][TWV]: the TwSet of every residue rho
   int n_t, n_chan, n_ant, n_pol, n_planes;
   int R, Cc;                 // occupied rows / columns of the block
   int nb;                    // batches per unit
@@ -185,12 +166,14 @@ __device__ __forceinline__ float biased_byte_to_float_bits(uint32_t w, int i) {
 }
 
 // word pair (lo plane, hi plane) of antennas a0..a0+3 -> E[a0..a0+3] = (re_lo, re_hi, im_lo, im_hi)
-__device__ __forceinline__ void unpack_words(uint32_t wlo, uint32_t whi, float4* __restrict__ e) {
+__device__ __forceinline__ void unpack_words(uint32_t wlo, uint32_t whi, float4* __restrict__ e, int rot) {
   const uint32_t rl = ((wlo >> 4) & 0x0F0F0F0Fu) ^ 0x08080808u, il = (wlo & 0x0F0F0F0Fu) ^ 0x08080808u;
   const uint32_t rh = ((whi >> 4) & 0x0F0F0F0Fu) ^ 0x08080808u, ih = (whi & 0x0F0F0F0Fu) ^ 0x08080808u;
   const float2 bias = f2(-12582920.0f);
 #pragma unroll
-  for (int i = 0; i < 4; ++i) {
+  for (int k = 0; k < 4; ++k) {
+    // lanes store their four cells in rotated order so that a quarter-warp covers all 8 bank groups
+    const int i = (k + rot) & 3;
     const float2 re = __fadd2_rn(make_float2(biased_byte_to_float_bits(rl, i), biased_byte_to_float_bits(rh, i)), bias);
     const float2 im = __fadd2_rn(make_float2(biased_byte_to_float_bits(il, i), biased_byte_to_float_bits(ih, i)), bias);
     e[i] = make_float4(re.x, re.y, im.x, im.y);
@@ -238,7 +221,7 @@ __device__ __forceinline__ void unpack_batch(const FusedParams& P, const Prefetc
                                              const uint32_t (&wlo)[MAXW], const uint32_t (&whi)[MAXW]) {
 #pragma unroll
   for (int k = 0; k < MAXW; ++k)
-    if (ps.j[k] >= 0) unpack_words(wlo[k], whi[k], E + ps.j[k] * P.n_ant + ps.a[k]);
+    if (ps.j[k] >= 0) unpack_words(wlo[k], whi[k], E + ps.j[k] * P.n_ant + ps.a[k], (int)(threadIdx.x >> 1));
 }
 
 // S3 for the batch: every thread owns the block cells tid + j*NT and sums their gather lists,
@@ -287,12 +270,9 @@ __device__ __forceinline__ void gather_batch(const FusedParams& P, const float4*
 // The caller guarantees both h-threads of a row sit in one warp and separates loads from stores
 // with __syncwarp().
 template <int NB>
-__device__ __forceinline__ void row_task(float4* __restrict__ row, const float4* __restrict__ tw, int tws,
-                                         int h, bool valid) {
+__device__ __forceinline__ void row_task(float4* __restrict__ row, const float4* __restrict__ tw, int h, bool valid) {
   C2 z[16];
-  const float4 c = tw[16 * tws];
-  fold_ramp<NB, 0>(z, row, 1, tw, tws, make_float2(c.x, c.y), make_float2(c.z, c.w));
-  fft16(z);
+  transform32<NB>(z, row, 1, tw);
   __syncwarp();
   if (valid) {
 #pragma unroll
@@ -303,12 +283,10 @@ __device__ __forceinline__ void row_task(float4* __restrict__ row, const float4*
 // columns + S5 + S6: thread = (l1, rho); outputs m = 2Q k + rho, k = 0..15.
 // acc[k] = (|A_lo|^2, |A_hi|^2) sums; xy[k] = sum of A_lo conj(A_hi) (reading Q11) when NPROD == 4.
 template <int NB, int NPROD>
-__device__ __forceinline__ void col_task(const float4* __restrict__ col, const float4* __restrict__ tw, int tws,
-                                         float2 cr, float2 ci, float2 (&acc)[16],
-                                         float2 (&xy)[NPROD == 4 ? 16 : 1]) {
+__device__ __forceinline__ void col_task(const float4* __restrict__ col, const float4* __restrict__ tw,
+                                         float2 (&acc)[16], float2 (&xy)[NPROD == 4 ? 16 : 1]) {
   C2 z[16];
-  fold_ramp<NB, 0>(z, col, HS, tw, tws, cr, ci);
-  fft16(z);
+  transform32<NB>(z, col, HS, tw);
 #pragma unroll
   for (int k = 0; k < 16; ++k) {
     acc[k] = __ffma2_rn(z[k].re, z[k].re, acc[k]);
@@ -323,11 +301,11 @@ __device__ __forceinline__ void col_task(const float4* __restrict__ col, const f
 template <int Q, int NPROD, bool DELTA, int NB>
 __global__ void __launch_bounds__(64 * Q, NPROD == 4 ? 1 : 2)
 epic_fused_kernel(FusedParams P) {
-  constexpr int NT = 64 * Q, N = 32 * Q, TWS = 2 * Q;
+  constexpr int NT = 64 * Q, N = 32 * Q;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* gh = reinterpret_cast<float4*>(smem_raw);  // [F][32][HS]
-  float4* tws = gh + F * PLANE;                      // [17][2Q]
-  float4* E = tws + 17 * TWS;                        // [F][A]
+  float4* tws = gh + F * PLANE;                      // [2Q][TWV]
+  float4* E = tws + 2 * Q * TWV;                     // [F][A]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
   // static, contiguous share of the (unit-major, batch-minor) work list
@@ -339,14 +317,14 @@ epic_fused_kernel(FusedParams P) {
 #pragma unroll
   for (int j = 0; j < S * S / NT; ++j) info[j] = __ldg(P.cell_info + tid + j * NT);
   for (int i = tid; i < F * PLANE; i += NT) gh[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);  // rows >= R stay zero
-  for (int i = tid; i < 17 * TWS; i += NT) tws[i] = __ldg(P.tw + i);
+  for (int i = tid; i < 2 * Q * TWV; i += NT) tws[i] = __ldg(P.tw + i);
   __syncthreads();
 
-  // column role: 8 consecutive l1 x 4 residues per warp (a warp reads 128 contiguous bytes per row)
-  const int l1 = (warp & 3) * 8 + (lane & 7);
-  const int rho = (warp >> 2) * 4 + (lane >> 3);
-  const float4 c_col = tws[16 * TWS + rho];
-  const float2 cr_c = make_float2(c_col.x, c_col.y), ci_c = make_float2(c_col.z, c_col.w);
+  // column role: 16 consecutive l1 x 2 residues per warp, the two residues of a column in ADJACENT
+  // lanes: LDS.128 merges same-address lane pairs, so a warp's load of a row is 2 wavefronts for
+  // 256 unique bytes (measured; lanes i and i+8 sharing an address do not merge: 4 wavefronts)
+  const int l1 = (warp & 1) * 16 + (lane >> 1);
+  const int rho = (warp >> 1) * 2 + (lane & 1);
 
   float2 acc[16];
   float2 xy[NPROD == 4 ? 16 : 1];
@@ -405,17 +383,17 @@ epic_fused_kernel(FusedParams P) {
       // idle lanes transform the all-zero row 31 of plane 0 (never written: they exist only when R < 32)
       int f = 0, y = S - 1, h = 0;
       if (valid) { h = task & 1; const int p = task >> 1; f = p / P.R; y = p - f * P.R; }
-      row_task<NB>(gh + f * PLANE + y * HS, tws + (l2 + Q * h), TWS, h, valid);
+      row_task<NB>(gh + f * PLANE + y * HS, tws + (l2 + Q * h) * TWV, h, valid);
     }
     __syncthreads();
 
     if (more) unpack_batch(P, ps, E, wlo, whi);  // E was last read by this batch's gather
 #pragma unroll 1
     for (int f = 0; f < F; ++f) {
-      // launder the table pointer: the 15 twiddles must be re-read per task, not held in 60 registers
-      int tw_off = rho;
+      // launder the table offset: the twiddles are re-read per task, not held in 18 registers
+      int tw_off = rho * TWV;
       asm volatile("" : "+r"(tw_off));
-      col_task<NB, NPROD>(gh + f * PLANE + l1, tws + tw_off, TWS, cr_c, ci_c, acc, xy);
+      col_task<NB, NPROD>(gh + f * PLANE + l1, tws + tw_off, acc, xy);
     }
 
     if (unit_n != unit || !more) flush(unit);
@@ -431,7 +409,7 @@ struct FusedTables {
 
 template <int Q>
 size_t fused_smem_bytes(int n_ant) {
-  return ((size_t)F * PLANE + (size_t)17 * 2 * Q + (size_t)F * n_ant) * sizeof(float4);
+  return ((size_t)F * PLANE + (size_t)2 * Q * TWV + (size_t)F * n_ant) * sizeof(float4);
 }
 
 template <int Q, int NPROD, bool DELTA, int NB>
@@ -488,15 +466,23 @@ int fused_plan_init(epic_plan* p) {
     if (c.ent_count > 255u) return EPIC_OK;  // falls back to the two-pass path
     info[(size_t)c.y * S + c.x] = (c.ent_begin << 8) | c.ent_count;
   }
-  // ramp table exp(+2 pi i y rho / N), y = 0..16, rho = 0..2Q-1, from double (reading Q8: + sign)
-  std::vector<float4> tw((size_t)17 * 2 * Q);
-  for (int y = 0; y <= 16; ++y)
-    for (int rho = 0; rho < 2 * Q; ++rho) {
-      const int ex = (y * rho) % p->N;
-      const double ang = 2.0 * M_PI * (double)ex / (double)p->N;
-      const float wr = (float)std::cos(ang), wi = (float)std::sin(ang);
-      tw[(size_t)y * 2 * Q + rho] = make_float4(wr, wr, wi, wi);
-    }
+  // TwSet of every residue rho = 0..2Q-1, from double (reading Q8: + sign): r = exp(2 pi i rho / N)
+  std::vector<float4> tw((size_t)2 * Q * TWV);
+  for (int rho = 0; rho < 2 * Q; ++rho) {
+    auto cis = [&](double r_pow, int k, int n, float* re, float* im) {  // r^r_pow W_n^k
+      const double ang = 2.0 * M_PI * ((double)rho * r_pow / (double)p->N + (double)k / (double)n);
+      *re = (float)std::cos(ang);
+      *im = (float)std::sin(ang);
+    };
+    float v[20] = {0};
+    cis(16.0, 0, 1, &v[0], &v[1]);                                       // fold: r^16
+    cis(8.0, 0, 2, &v[2], &v[3]);                                        // level 2
+    cis(4.0, 0, 4, &v[4], &v[5]);                                        // level 4
+    for (int k = 0; k < 2; ++k) cis(2.0, k, 8, &v[6 + 2 * k], &v[7 + 2 * k]);    // level 8
+    for (int k = 0; k < 4; ++k) cis(1.0, k, 16, &v[10 + 2 * k], &v[11 + 2 * k]);  // level 16
+    for (int j = 0; j < TWV; ++j)
+      tw[(size_t)rho * TWV + j] = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+  }
   FusedTables* ft = new (std::nothrow) FusedTables();
   if (!ft) return EPIC_ERR_NOMEM;
   ft->cell_info = nullptr;
