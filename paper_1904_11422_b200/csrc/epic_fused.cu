@@ -147,7 +147,8 @@ __device__ __forceinline__ void transform32(C2 (&z)[16], const float4* __restric
 struct FusedParams {
   const uint8_t* volt;       // [T][C][NPOL][A] 4+4-bit samples
   float* out;                // [C][planes][N][N]
-  const uint32_t* cell_info; // [32*32] dense block cells: (first entry << 8) | entry count
+  const uint2* cell_info;    // [32*32] cell slots sorted by entry count: x = (first entry << 8) | count,
+                             // y = cell offset cy*HS + cx in a plane (0xFFFFFFFF: unused slot)
   const uint16_t* ent_ant;   // gather entries, sorted by block cell
   const float2* ent_tap;
   const float4* tw;          // [2Q][TWV]: the TwSet of every residue rho
@@ -224,17 +225,17 @@ __device__ __forceinline__ void unpack_batch(const FusedParams& P, const Prefetc
     if (ps.j[k] >= 0) unpack_words(wlo[k], whi[k], E + ps.j[k] * P.n_ant + ps.a[k], (int)(threadIdx.x >> 1));
 }
 
-// S3 for the batch: every thread owns the block cells tid + j*NT and sums their gather lists,
-// in table order, for all F pair-planes (collisions sum).
+// S3 for the batch: every thread owns the cell slots tid + j*NT of the plan's list and sums their
+// gather lists, in table order, for all F pair-planes (collisions sum).  The
+// list holds every cell of the R x 32 block (empty ones are written as zeros) sorted by entry
+// count, so the 32 cells of a warp have (nearly) equal trip counts.
 template <int NT, bool DELTA>
 __device__ __forceinline__ void gather_batch(const FusedParams& P, const float4* __restrict__ E,
-                                             float4* __restrict__ gh, const uint32_t (&info)[S * S / NT], int tid) {
+                                             float4* __restrict__ gh, const uint2 (&info)[S * S / NT]) {
 #pragma unroll
   for (int j = 0; j < S * S / NT; ++j) {
-    const int cell = tid + j * NT;
-    const int cy = cell >> 5, cx = cell & 31;
-    if (cy >= P.R) continue;
-    const uint32_t beg = info[j] >> 8, cnt = info[j] & 0xFFu;
+    if (info[j].y == 0xFFFFFFFFu) continue;
+    const uint32_t beg = info[j].x >> 8, cnt = info[j].x & 0xFFu;
     float2 sr[F], si[F];
 #pragma unroll
     for (int f = 0; f < F; ++f) { sr[f] = make_float2(0.0f, 0.0f); si[f] = make_float2(0.0f, 0.0f); }
@@ -259,7 +260,7 @@ __device__ __forceinline__ void gather_batch(const FusedParams& P, const float4*
         }
       }
     }
-    float4* dst = gh + cy * HS + cx;
+    float4* dst = gh + info[j].y;
 #pragma unroll
     for (int f = 0; f < F; ++f) dst[f * PLANE] = make_float4(sr[f].x, sr[f].y, si[f].x, si[f].y);
   }
@@ -313,7 +314,7 @@ epic_fused_kernel(FusedParams P) {
   const long long g1 = P.total * (long long)(blockIdx.x + 1) / gridDim.x;
   if (g0 >= g1) return;
 
-  uint32_t info[S * S / NT];
+  uint2 info[S * S / NT];
 #pragma unroll
   for (int j = 0; j < S * S / NT; ++j) info[j] = __ldg(P.cell_info + tid + j * NT);
   for (int i = tid; i < F * PLANE; i += NT) gh[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);  // rows >= R stay zero
@@ -373,7 +374,7 @@ epic_fused_kernel(FusedParams P) {
     const bool more = g + 1 < g1;
     if (more) prefetch_batch<NT>(P, ps, unit_n / Q, b_n, wlo, whi);
 
-    gather_batch<NT, DELTA>(P, E, gh, info, tid);
+    gather_batch<NT, DELTA>(P, E, gh, info);
     __syncthreads();
 
     const int l2 = unit % Q;
@@ -403,7 +404,7 @@ epic_fused_kernel(FusedParams P) {
 }
 
 struct FusedTables {
-  uint32_t* cell_info;
+  uint2* cell_info;
   float4* tw;
 };
 
@@ -461,11 +462,19 @@ int fused_plan_init(epic_plan* p) {
   if (p->N % S != 0 || (Q != 2 && Q != 4)) return EPIC_OK;
   if (p->R > S || p->Cc > S) return EPIC_OK;
   if (p->h_ent_ant.size() >= ((size_t)1 << 24)) return EPIC_OK;
-  std::vector<uint32_t> info((size_t)S * S, 0u);
+  std::vector<uint32_t> dense((size_t)S * S, 0u);
   for (const CellRec& c : p->h_cells) {
     if (c.ent_count > 255u) return EPIC_OK;  // falls back to the two-pass path
-    info[(size_t)c.y * S + c.x] = (c.ent_begin << 8) | c.ent_count;
+    dense[(size_t)c.y * S + c.x] = (c.ent_begin << 8) | c.ent_count;
   }
+  // every cell of the R x 32 block (columns >= Cc are re-zeroed each batch: the row pass writes
+  // its output in place), sorted by entry count so that warps see uniform trip counts
+  std::vector<uint2> info;
+  for (int y = 0; y < p->R; ++y)
+    for (int x = 0; x < S; ++x) info.push_back(make_uint2(dense[(size_t)y * S + x], (uint32_t)(y * HS + x)));
+  std::stable_sort(info.begin(), info.end(),
+                   [](const uint2& l, const uint2& r) { return (l.x & 0xFFu) > (r.x & 0xFFu); });
+  info.resize((size_t)S * S, make_uint2(0u, 0xFFFFFFFFu));
   // TwSet of every residue rho = 0..2Q-1, from double (reading Q8: + sign): r = exp(2 pi i rho / N)
   std::vector<float4> tw((size_t)2 * Q * TWV);
   for (int rho = 0; rho < 2 * Q; ++rho) {
@@ -487,10 +496,10 @@ int fused_plan_init(epic_plan* p) {
   if (!ft) return EPIC_ERR_NOMEM;
   ft->cell_info = nullptr;
   ft->tw = nullptr;
-  cudaError_t ce = cudaMalloc(&ft->cell_info, info.size() * sizeof(uint32_t));
+  cudaError_t ce = cudaMalloc(&ft->cell_info, info.size() * sizeof(uint2));
   if (ce == cudaSuccess) ce = cudaMalloc(&ft->tw, tw.size() * sizeof(float4));
   if (ce == cudaSuccess)
-    ce = cudaMemcpy(ft->cell_info, info.data(), info.size() * sizeof(uint32_t), cudaMemcpyHostToDevice);
+    ce = cudaMemcpy(ft->cell_info, info.data(), info.size() * sizeof(uint2), cudaMemcpyHostToDevice);
   if (ce == cudaSuccess) ce = cudaMemcpy(ft->tw, tw.data(), tw.size() * sizeof(float4), cudaMemcpyHostToDevice);
   if (ce != cudaSuccess) {
     set_cuda_error(ce);
