@@ -18,22 +18,23 @@
 //
 // Work unit = (channel c, column residue l2); its CTA owns the image columns l = Q l1 + l2 and
 // keeps their accumulators in registers for the unit's whole time range.  One 32-point transform
-// with ramp is split over two threads h = 0,1 (outputs 2k + h):
+// with residue rho is split over two threads h = 0,1 (outputs m1 = 2k + h):
 //
-//   X[2Q k + rho] = sum_{y<16} [ (in[y] + (-1)^h in[y+16]) W_N^{y rho} ] W_16^{y k},  rho = r + Q h,
+//   X[2Q k + rho'] = sum_{y<16} (in[y] + r^16 in[y+16]) r^y W_16^{y k},  rho' = rho + Q h,  r = W_N^{rho'}
 //
-// i.e. fold, multiply by a table twiddle, 16-point radix-2 FFT with immediate twiddles.  Rows
-// (along x, r = l2) and columns (along y, r = m2) run the SAME code, so the hot loop is a few KB
-// of instructions shared by all warps (the first version of this kernel unrolled every residue
-// separately, 109 KB of code, and was instruction-fetch bound: profiles/r01_fused_v1_*).
+// i.e. a fold and a 16-point radix-2 FFT whose twiddles carry the ramp r^y (nine per-residue
+// complex numbers read from shared memory; see TwSet).  Rows (along x, rho = l2) and columns
+// (along y, rho = m2) run the SAME code, so the hot loop is a few KB of instructions shared by
+// all warps.  (The first version of this kernel unrolled every residue with immediate twiddles:
+// 109 KB of code, instruction-fetch bound at 0.36 of the roofline; profiles/r01_fused_history.md.)
 //
 //   per batch of F pairs (F time samples when n_pol == 2):
 //     prefetch  next batch's 4+4-bit voltages, global -> registers (consumed one batch later)
-//     gather    S3: every thread owns fixed cells of the 32x32 block and sums its (antenna, tap)
+//     gather    S3: every thread owns fixed cells of the R x 32 block and sums its (antenna, tap)
 //               list in table order from the unpacked voltages E (no atomics, deterministic)
 //     rows      S4 along x, thread = (pair, row y, h), in place
 //     unpack    S1: the prefetched words -> E (float4 per antenna) for the NEXT batch
-//     columns   S4 along y + S5 + S6: thread = (l1, rho); 16 outputs -> products -> += registers
+//     columns   S4 along y + S5 + S6: thread = (l1, rho'); 16 outputs -> products -> += registers
 //   at the end of the unit's time range: one add per pixel into out_accum.
 #include <algorithm>
 
@@ -47,7 +48,7 @@ constexpr int HS = 34;       // row stride of a shared plane in float4 cells (ba
 constexpr int PLANE = S * HS;  // float4 cells per pair-plane
 constexpr int F = 4;         // pairs per batch
 constexpr int MAXW = 2;      // prefetched word pairs per thread
-constexpr int CHUNK = 2;     // fold_ramp: elements whose loads may be in flight together
+constexpr int CHUNK = 2;     // fold: elements whose loads may be in flight together
 
 constexpr int TWV = 5;       // float4 words of twiddles per residue (TwSet)
 
