@@ -31,6 +31,8 @@ METRIC = "E-field frames/sec (chan x time gridded+FFT'd+accumulated)"
 UNIT = "frames/s"
 FP32_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # SMs x lanes x FMA x max clock
 L2_FLUSH_BYTES = 256 << 20
+PATH_NAMES = {1: "twopass", 2: "fused", 3: "tiled"}
+PATH_KERNELS = {1: "grid_rowfft+colfft_accum", 2: "epic_fused_kernel", 3: "tiled_rows+tiled_cols"}
 
 
 def algorithmic_flops_per_frame(wl) -> float:
@@ -179,7 +181,7 @@ def run_epic(args, wl):
     plan = epic.Plan(wl.grid_n, wl.pad, wl.ant_uv, wl.taps, wl.kernel_k)
     plan.set_products(wl.n_products)
     if args.path:
-        plan.set_path({"auto": 0, "twopass": 1, "fused": 2}[args.path])
+        plan.set_path({"auto": 0, "twopass": 1, "fused": 2, "tiled": 3}[args.path])
     planes = plan.n_planes(wl.n_pol)
     out = torch.zeros((wl.n_chan, planes, wl.N, wl.N), dtype=torch.float32, device=dev)
     h_out = torch.empty(out.shape, dtype=torch.float32).pin_memory()
@@ -254,7 +256,7 @@ def run_epic(args, wl):
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         try:
-            traffic = json.load(open(tpath)).get(f"{wl.name}:{'fused' if path == 2 else 'twopass'}")
+            traffic = json.load(open(tpath)).get(f"{wl.name}:{PATH_NAMES.get(path)}")
         except (OSError, ValueError):
             traffic = None
     line = {
@@ -262,7 +264,7 @@ def run_epic(args, wl):
         "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": wl.name, **{k: v for k, v in wl.describe().items() if k != "workload"},
-                   "kernel_path": {1: "twopass", 2: "fused"}.get(path, str(path)),
+                   "kernel_path": PATH_NAMES.get(path, str(path)),
                    "support_box": list(support), "l2": f"flushed between iterations ({L2_FLUSH_BYTES >> 20} MiB write)",
                    "sharding": "independent replicas of the workload per GPU (channels are independent), no collective"},
         "roofline": {
@@ -293,7 +295,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (1-based)")
     ap.add_argument("--impl", default="epic", choices=["epic", "reference"])
-    ap.add_argument("--path", default=None, choices=[None, "auto", "twopass", "fused"])
+    ap.add_argument("--path", default=None, choices=[None, "auto", "twopass", "fused", "tiled"])
     ap.add_argument("--n-chan", type=int, default=None)
     ap.add_argument("--n-t", type=int, default=None)
     ap.add_argument("--n-ant", type=int, default=None)

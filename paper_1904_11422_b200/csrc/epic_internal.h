@@ -42,6 +42,8 @@ struct epic_plan {
   size_t scratch_bytes;
   void* d_fused;               // tables private to the fused path
   int fused_ok;                // support fits the fused kernel
+  void* d_tiled;               // tables private to the tiled path
+  int tiled_ok;                // N is 256 or 512
   int n_sm;
   // host copies kept for the fused path's table builder
   std::vector<epic::CellRec> h_cells;
@@ -70,6 +72,12 @@ int fused_plan_init(epic_plan* p);  // sets p->fused_ok, allocates p->d_fused
 void fused_plan_free(epic_plan* p);
 int fused_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products);
 int fused_image(epic_plan* p, const ImageArgs& a);
+
+// epic_tiled.cu
+int tiled_plan_init(epic_plan* p);  // sets p->tiled_ok, allocates p->d_tiled
+void tiled_plan_free(epic_plan* p);
+int tiled_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products);
+int tiled_image(epic_plan* p, const ImageArgs& a);
 
 void set_cuda_error(cudaError_t e);
 

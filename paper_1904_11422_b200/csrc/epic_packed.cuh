@@ -1,0 +1,112 @@
+// Device helpers shared by the packed (f32x2) kernels: epic_fused.cu and epic_tiled.cu.
+//
+// Every complex value is carried as a PAIR of planes in the two halves of f32x2 registers
+// (sm_100 FFMA2/FADD2: one issue slot, two FP32 lanes; the twiddle is one broadcast .F32 operand):
+// (lo, hi) = (pol X, pol Y) of one time sample when n_pol == 2, or two consecutive time samples
+// when n_pol == 1.  A shared/global memory cell is a float4 (re_lo, re_hi, im_lo, im_hi).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace epic {
+namespace {
+
+constexpr int TWV = 5;       // float4 words of twiddles per residue (TwSet)
+
+// ---------------------------------------------------------------- packed complex pair
+struct C2 { float2 re, im; };  // (lo, hi) halves = two independent planes
+
+__device__ __forceinline__ float2 f2(float v) { return make_float2(v, v); }  // FFMA2 takes it as one .F32 operand
+__device__ __forceinline__ float2 neg2(float2 v) { return make_float2(-v.x, -v.y); }
+
+// The transform one thread computes (rows and columns alike):
+//
+//   X[k] = sum_{y<32} in[y] r^y W_16^{y k},  k = 0..15,   r = W_N^{rho}  (|r| = 1)
+//        = sum_{y<16} (in[y] + r^16 in[y+16]) r^y W_16^{y k}
+//
+// The residue ramp r^y is absorbed into the butterflies: decimation in time gives, for a length-n
+// sub-transform T_n(s, r_n),  T_n[k], T_n[k + n/2] = T_{n/2}(s_even, r_n^2)[k] +- (r_n W_n^k) T_{n/2}(s_odd, r_n^2)[k],
+// so level n = 2, 4, 8, 16 uses the twiddles r^{16/n} W_n^k: nine complex numbers per residue
+// (W_n^{k + n/4} = i W_n^k is a register swap), computed in double on the host.
+struct TwSet {
+  float cr, ci;              // r^16        (fold)
+  float w2r, w2i;            // r^8         (level 2)
+  float w4r, w4i;            // r^4         (level 4, k = 0; k = 1 is i times it)
+  float w8r[2], w8i[2];      // r^2 W_8^k   (level 8, k = 0, 1)
+  float w16r[4], w16i[4];    // r W_16^k    (level 16, k = 0..3)
+};
+
+// shared-memory image of a TwSet: TWV float4 words
+//   [0] = (cr, ci, w2r, w2i)  [1] = (w4r, w4i, w8r0, w8i0)  [2] = (w8r1, w8i1, w16r0, w16i0)
+//   [3] = (w16r1, w16i1, w16r2, w16i2)  [4] = (w16r3, w16i3, 0, 0)
+
+// radix-2 DIT butterfly on packed pairs: (a, b) <- (a + w b, a - w b); 6 FFMA2
+__device__ __forceinline__ void bfly(C2& a, C2& b, float wr, float wi) {
+  C2 p;
+  p.re = __ffma2_rn(b.re, f2(wr), a.re); p.re = __ffma2_rn(neg2(b.im), f2(wi), p.re);
+  p.im = __ffma2_rn(b.im, f2(wr), a.im); p.im = __ffma2_rn(b.re, f2(wi), p.im);
+  b.re = __ffma2_rn(a.re, f2(2.0f), neg2(p.re));
+  b.im = __ffma2_rn(a.im, f2(2.0f), neg2(p.im));
+  a = p;
+}
+// the same with twiddle i w = (-wi, wr)
+__device__ __forceinline__ void bfly_i(C2& a, C2& b, float wr, float wi) { bfly(a, b, -wi, wr); }
+
+// z holds s[y] = in[y] + r^16 in[y+16] in bit-reversed order; on return z[k] = X[k].
+// Twiddles are read from the residue's shared-memory TwSet level by level (short live ranges).
+__device__ __forceinline__ void fft16_ramped(C2 (&z)[16], const float4* __restrict__ tw, float w2r, float w2i) {
+#pragma unroll
+  for (int b = 0; b < 16; b += 2) bfly(z[b], z[b + 1], w2r, w2i);
+  const float4 t1 = tw[1];
+#pragma unroll
+  for (int b = 0; b < 16; b += 4) { bfly(z[b], z[b + 2], t1.x, t1.y); bfly_i(z[b + 1], z[b + 3], t1.x, t1.y); }
+  const float4 t2 = tw[2];
+#pragma unroll
+  for (int b = 0; b < 16; b += 8) {
+    bfly(z[b], z[b + 4], t1.z, t1.w);   bfly(z[b + 1], z[b + 5], t2.x, t2.y);
+    bfly_i(z[b + 2], z[b + 6], t1.z, t1.w); bfly_i(z[b + 3], z[b + 7], t2.x, t2.y);
+  }
+  const float4 t3 = tw[3], t4 = tw[4];
+  bfly(z[0], z[8], t2.z, t2.w);    bfly(z[1], z[9], t3.x, t3.y);
+  bfly(z[2], z[10], t3.z, t3.w);   bfly(z[3], z[11], t4.x, t4.y);
+  bfly_i(z[4], z[12], t2.z, t2.w); bfly_i(z[5], z[13], t3.x, t3.y);
+  bfly_i(z[6], z[14], t3.z, t3.w); bfly_i(z[7], z[15], t4.x, t4.y);
+}
+
+// 8-point version: z holds the input in 3-bit bit-reversed order; twiddles (base q):
+// q^4 (level 2), q^2 (level 4; k = 1 is i times it), q W_8^k, k = 0, 1 (level 8).
+__device__ __forceinline__ void fft8_ramped(C2 (&z)[8], float w2r, float w2i, float w4r, float w4i,
+                                            float w80r, float w80i, float w81r, float w81i) {
+#pragma unroll
+  for (int b = 0; b < 8; b += 2) bfly(z[b], z[b + 1], w2r, w2i);
+#pragma unroll
+  for (int b = 0; b < 8; b += 4) { bfly(z[b], z[b + 2], w4r, w4i); bfly_i(z[b + 1], z[b + 3], w4r, w4i); }
+  bfly(z[0], z[4], w80r, w80i);   bfly(z[1], z[5], w81r, w81i);
+  bfly_i(z[2], z[6], w80r, w80i); bfly_i(z[3], z[7], w81r, w81i);
+}
+
+// S1 (reading Q1).  Four samples per 32-bit word: high nibbles are the real
+// parts, low nibbles the imaginary parts, two's complement.  n ^ 8 = sext4(n) + 8 in 0..15;
+// dropping that byte into the mantissa of 12582912.0f (0x4B400000) and subtracting 12582920.0f
+// gives sext4(n) exactly, with no integer-to-float conversion instruction.
+__device__ __forceinline__ float biased_byte_to_float_bits(uint32_t w, int i) {
+  return __uint_as_float(__byte_perm(w, 0x4B400000u, 0x7650u + (uint32_t)i));
+}
+
+// word pair (lo plane, hi plane) of antennas a0..a0+3 -> E[a0..a0+3] = (re_lo, re_hi, im_lo, im_hi)
+__device__ __forceinline__ void unpack_words(uint32_t wlo, uint32_t whi, float4* __restrict__ e, int rot) {
+  const uint32_t rl = ((wlo >> 4) & 0x0F0F0F0Fu) ^ 0x08080808u, il = (wlo & 0x0F0F0F0Fu) ^ 0x08080808u;
+  const uint32_t rh = ((whi >> 4) & 0x0F0F0F0Fu) ^ 0x08080808u, ih = (whi & 0x0F0F0F0Fu) ^ 0x08080808u;
+  const float2 bias = f2(-12582920.0f);
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    // lanes store their four cells in rotated order so that a quarter-warp covers all 8 bank groups
+    const int i = (k + rot) & 3;
+    const float2 re = __fadd2_rn(make_float2(biased_byte_to_float_bits(rl, i), biased_byte_to_float_bits(rh, i)), bias);
+    const float2 im = __fadd2_rn(make_float2(biased_byte_to_float_bits(il, i), biased_byte_to_float_bits(ih, i)), bias);
+    e[i] = make_float4(re.x, re.y, im.x, im.y);
+  }
+}
+
+}  // namespace
+}  // namespace epic

@@ -187,14 +187,20 @@ static int image_common(epic_plan* plan, const void* volt, int is_cf32, int n_t,
   a.n_planes = n_planes;
   a.out = out;
   a.stream = (cudaStream_t)stream;
+  const int tiled_can = tiled_supported(plan, is_cf32, n_pol, n_products) &&
+                        (reinterpret_cast<uintptr_t>(volt) & 3u) == 0;
   int path = plan->path_req;
   // the fused kernel reads voltage rows as 32-bit words
   const int fused_can = fused_supported(plan, is_cf32, n_pol, n_products) &&
                         (reinterpret_cast<uintptr_t>(volt) & 3u) == 0;
-  if (path == EPIC_PATH_AUTO) path = fused_can ? EPIC_PATH_FUSED : EPIC_PATH_TWOPASS;
+  if (path == EPIC_PATH_AUTO) path = fused_can ? EPIC_PATH_FUSED : (tiled_can ? EPIC_PATH_TILED : EPIC_PATH_TWOPASS);
   if (path == EPIC_PATH_FUSED) {
     if (!fused_can) return EPIC_ERR_RANGE;
     return fused_image(plan, a);
+  }
+  if (path == EPIC_PATH_TILED) {
+    if (!tiled_can) return EPIC_ERR_RANGE;
+    return tiled_image(plan, a);
   }
   return twopass_image(plan, a);
 }
@@ -234,6 +240,8 @@ int epic_plan_create(epic_plan** out, int grid_n, int pad, int n_ant, const floa
   p->d_scratch = nullptr;
   p->d_fused = nullptr;
   p->fused_ok = 0;
+  p->d_tiled = nullptr;
+  p->tiled_ok = 0;
   p->scratch_bytes = 0;
   int dev = 0;
   cudaDeviceProp prop;
@@ -254,7 +262,7 @@ int epic_plan_create(epic_plan** out, int grid_n, int pad, int n_ant, const floa
   if (st == EPIC_OK) {
     // two-pass intermediate: at least one dual-pol frame, otherwise an L2-sized ring
     const size_t frame = (size_t)2 * p->R * p->N * sizeof(float2);
-    p->scratch_bytes = std::max((size_t)64 << 20, frame);
+    p->scratch_bytes = std::max((size_t)96 << 20, frame);
     ce = cudaMalloc(&p->d_scratch, p->scratch_bytes);
     if (ce != cudaSuccess) {
       set_cuda_error(ce);
@@ -262,6 +270,7 @@ int epic_plan_create(epic_plan** out, int grid_n, int pad, int n_ant, const floa
     }
   }
   if (st == EPIC_OK) st = fused_plan_init(p);
+  if (st == EPIC_OK) st = tiled_plan_init(p);
   if (st != EPIC_OK) {
     epic_plan_destroy(p);
     return st;
@@ -274,6 +283,7 @@ int epic_plan_destroy(epic_plan* plan) {
   if (!plan) return EPIC_OK;
   cudaError_t ce = cudaDeviceSynchronize();
   fused_plan_free(plan);
+  tiled_plan_free(plan);
   if (plan->d_scratch) cudaFree(plan->d_scratch);
   if (plan->d_blob) cudaFree(plan->d_blob);
   delete plan;
@@ -293,8 +303,10 @@ int epic_plan_set_products(epic_plan* plan, int n_products) {
 
 int epic_plan_set_path(epic_plan* plan, int path) {
   if (!plan) return EPIC_ERR_ARG;
-  if (path != EPIC_PATH_AUTO && path != EPIC_PATH_TWOPASS && path != EPIC_PATH_FUSED) return EPIC_ERR_ARG;
+  if (path != EPIC_PATH_AUTO && path != EPIC_PATH_TWOPASS && path != EPIC_PATH_FUSED && path != EPIC_PATH_TILED)
+    return EPIC_ERR_ARG;
   if (path == EPIC_PATH_FUSED && !plan->fused_ok) return EPIC_ERR_RANGE;
+  if (path == EPIC_PATH_TILED && !plan->tiled_ok) return EPIC_ERR_RANGE;
   plan->path_req = path;
   return EPIC_OK;
 }
@@ -339,7 +351,8 @@ int epic_plan_get_path(const epic_plan* plan, int n_pol) {
   const int n_products = resolve_products(plan, n_pol);
   if (planes_for(n_pol, n_products) < 0) return EPIC_ERR_RANGE;
   if (plan->path_req != EPIC_PATH_AUTO) return plan->path_req;
-  return fused_supported(plan, 0, n_pol, n_products) ? EPIC_PATH_FUSED : EPIC_PATH_TWOPASS;
+  if (fused_supported(plan, 0, n_pol, n_products)) return EPIC_PATH_FUSED;
+  return tiled_supported(plan, 0, n_pol, n_products) ? EPIC_PATH_TILED : EPIC_PATH_TWOPASS;
 }
 
 int epic_plan_last_launches(const epic_plan* plan) { return plan ? plan->last_launches : (int)EPIC_ERR_ARG; }

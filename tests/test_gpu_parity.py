@@ -152,6 +152,45 @@ def test_fused_capable_plans_both_paths(wl, path):
             assert plan.path(wl.n_pol) == epic.EPIC_PATH_FUSED  # AUTO picks it
 
 
+# Large planes (N = 256, 512): the tiled (packed, L2-resident two-pass) path and the general
+# two-pass path must each match the oracle; AUTO must pick the tiled one.
+TILED_CAPABLE = [
+    make_config(4, n_chan=2, n_t=5),                                  # N = 256, prefold of 2 rows/cols
+    make_config(5, n_chan=1, n_t=3),                                  # N = 512, wrap-around box, 5x5 taps
+    make_config(5, n_chan=2, n_t=3, n_ant=256),
+    make_custom(grid_n=128, pad=2, n_ant=64, n_pol=2, kernel_k=1, n_chan=3, n_t=4, layout="disc",
+                n_products=2),                                        # small support: no prefold, zero rows
+    make_custom(grid_n=256, pad=1, n_ant=200, n_pol=2, kernel_k=3, n_chan=1, n_t=3, layout="uniform"),  # R = N
+    make_custom(grid_n=128, pad=2, n_ant=100, n_pol=1, kernel_k=3, n_chan=2, n_t=7, layout="uniform"),  # 1 pol, odd n_t
+    make_custom(grid_n=128, pad=4, n_ant=300, n_pol=2, kernel_k=1, n_chan=1, n_t=2, layout="wrap"),     # N = 512, delta
+    make_custom(grid_n=256, pad=2, n_ant=40, n_pol=1, kernel_k=1, n_chan=1, n_t=4, layout="uniform"),
+]
+
+
+@pytest.mark.parametrize("path", [1, 3], ids=["twopass", "tiled"])
+@pytest.mark.parametrize("wl", TILED_CAPABLE, ids=lambda w: f"{w.name}-c{w.n_chan}-t{w.n_t}")
+def test_tiled_capable_plans_both_paths(wl, path):
+    epic = _epic()
+    gpu, info = run_gpu(wl, path=path, return_plan_info=True)
+    assert info["path"] == path
+    ref = run_oracle(wl)
+    assert_parity(gpu, ref, what=f"{wl.name} path={path}")
+    if path == 3:
+        with epic.Plan(wl.grid_n, wl.pad, wl.ant_uv, wl.taps, wl.kernel_k) as plan:
+            plan.set_products(wl.n_products)
+            assert plan.path(wl.n_pol) == epic.EPIC_PATH_TILED  # AUTO picks it
+
+
+def test_tiled_many_batches_accumulate():
+    """More frames than one scratch batch holds, several channels: exercises the batch loop and
+    the one-add-per-batch accumulation of the column kernel."""
+    wl = make_config(4, n_chan=5, n_t=70)
+    gpu, info = run_gpu(wl, path=3, return_plan_info=True)
+    assert info["launches"] >= 4
+    ref = run_oracle(wl, channels=[0, 4])
+    assert_parity(gpu[[0, 4]], ref, what="C4 5ch x 70")
+
+
 def test_fused_delta_gridding_is_exact_for_integer_voltages():
     """Delta kernel + 4-bit integers: every gridded value is a small integer, so a one-antenna-
     per-pixel check through the whole fused path is exact: a single antenna gives a flat image
@@ -165,6 +204,24 @@ def test_fused_delta_gridding_is_exact_for_integer_voltages():
     for c in range(wl.n_chan):
         for p in range(2):
             assert np.all(gpu[c, p] == np.float32(flat[c, p]))
+
+
+# ------------------------------------------------------------------ full size, sampled outputs
+@pytest.mark.parametrize("idx,channels", [(2, [0, 77, 127]), (3, [5, 126])], ids=["C2-full", "C3-full"])
+def test_full_size_config_sampled_channels(idx, channels):
+    """BASELINE.json's C2 / C3 at full extent, in the launch configuration bench.py times (one
+    epic_image call over all channels and samples, AUTO path = fused); the oracle recomputes
+    whole channels picked across the range (channels are independent)."""
+    wl = make_config(idx)
+    v = wl.voltages()
+    gpu, info = run_gpu(wl, volt=v, return_plan_info=True)
+    assert info["path"] == 2 and info["launches"] == 1
+    ref = run_oracle(wl, volt=v, channels=channels)
+    assert_parity(gpu[channels], ref, what=f"{wl.name} channels {channels}")
+    # properties that hold for every channel at any size
+    assert np.isfinite(gpu).all() and (gpu[:, :2] >= 0).all()
+    totals = gpu[:, 0].sum(axis=(1, 2))
+    assert totals.min() > 0.5 * totals.max()  # every channel was imaged (same noise statistics)
 
 
 def test_calls_accumulate_into_out_accum():
