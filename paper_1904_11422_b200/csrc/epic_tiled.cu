@@ -37,6 +37,8 @@ constexpr int NT_B = 128;  // threads of tiled_cols
 constexpr int XJ = 17;     // exchange buffer: [team][j][XJ] float4, k1 < 16 (padded: conflict-free both ways)
 
 template <int J> constexpr int x_team_stride() { return ((J * XJ + 7) / 8) * 8 + 4; }  // = 4 mod 8
+// tiled_cols: a quarter-warp is 8 teams with one j, so consecutive teams must fall in distinct bank groups
+template <int J> constexpr int x_team_stride_cols() { return (J * XJ) | 1; }
 constexpr int bitrev3(int v) { return ((v & 1) << 2) | (v & 2) | ((v & 4) >> 2); }
 constexpr int bitrev4t(int v) { return ((v & 1) << 3) | ((v & 2) << 1) | ((v & 4) >> 1) | ((v & 8) >> 3); }
 
@@ -63,7 +65,8 @@ __device__ __forceinline__ C2 to_c2(float4 v) { return C2{make_float2(v.x, v.y),
 __device__ __forceinline__ float4 to_f4(const C2& z) { return make_float4(z.re.x, z.re.y, z.im.x, z.im.y); }
 
 // ---------------------------------------------------------------- kernel A: unpack, grid, row transforms
-// CTA = one frame pair (blockIdx.x) and every gridDim.y-th group of RG occupied rows.
+// Work item = (frame pair of the batch, group of RG occupied rows); every CTA takes an equal contiguous
+// range of items (one wave, no tail) and re-unpacks E when its frame changes.
 // Thread roles in the transform steps: tid = rho + 2 j + 2 J r  (row r of the group, team (r, rho)).
 // One shared buffer BUF serves in turn as the gridded rows RB[RG][N], the exchange buffer
 // X[team][j][XJ] and the transformed rows; registers carry the data across the hand-overs.
@@ -78,28 +81,33 @@ __global__ void __launch_bounds__(NT_A) tiled_rows(TiledParams P) {
   float4* E = tw2 + 2 * 16 * TWV;                     // [A]
   const int tid = threadIdx.x;
   const DevTables& t = P.t;
-  const int fb = blockIdx.x, cb = fb / P.Tb, pb = fb - cb * P.Tb;
-  const int c = P.c0 + cb, pair = P.p0 + pb;
-
   for (int i = tid; i < 2 * TWV; i += NT_A) tw1[i] = __ldg(P.tw1 + i);
   for (int i = tid; i < 2 * 16 * TWV; i += NT_A) tw2[i] = __ldg(P.tw2 + i);
-  {  // S1: this frame pair's voltages -> E
-    const int t_lo = P.n_pol == 2 ? pair : 2 * pair, t_hi = P.n_pol == 2 ? pair : 2 * pair + 1;
-    const size_t row_bytes = (size_t)P.n_pol * t.n_ant;
-    const uint8_t* lo = P.volt + ((size_t)t_lo * P.n_chan + c) * row_bytes;
-    const uint8_t* hi = P.volt + ((size_t)t_hi * P.n_chan + c) * row_bytes + (P.n_pol == 2 ? t.n_ant : 0);
-    for (int g = tid; g < (t.n_ant >> 2); g += NT_A) {
-      const uint32_t wlo = t_lo < P.n_t ? __ldg(reinterpret_cast<const uint32_t*>(lo) + g) : 0u;
-      const uint32_t whi = t_hi < P.n_t ? __ldg(reinterpret_cast<const uint32_t*>(hi) + g) : 0u;
-      unpack_words(wlo, whi, E + 4 * g, tid >> 1);
-    }
-  }
-  __syncthreads();
 
   const int rho = tid & 1, j = (tid >> 1) & (J - 1), r = tid / (2 * J);
   float4* xt = buf + (2 * r + rho) * XS;  // this team's exchange block
   const int n_groups = (t.R + RG - 1) / RG;
-  for (int g = blockIdx.y; g < n_groups; g += gridDim.y) {
+  const long long n_items = (long long)P.Cb * P.Tb * n_groups;
+  const int item0 = (int)(n_items * blockIdx.x / gridDim.x), item1 = (int)(n_items * (blockIdx.x + 1) / gridDim.x);
+  int fb_loaded = -1;
+  for (int item = item0; item < item1; ++item) {
+    const int fb = item / n_groups, g = item - fb * n_groups;
+    if (fb != fb_loaded) {  // S1: this frame pair's voltages -> E
+      fb_loaded = fb;
+      const int cb = fb / P.Tb, pb = fb - cb * P.Tb;
+      const int c = P.c0 + cb, pair = P.p0 + pb;
+      const int t_lo = P.n_pol == 2 ? pair : 2 * pair, t_hi = P.n_pol == 2 ? pair : 2 * pair + 1;
+      const size_t row_bytes = (size_t)P.n_pol * t.n_ant;
+      const uint8_t* lo = P.volt + ((size_t)t_lo * P.n_chan + c) * row_bytes;
+      const uint8_t* hi = P.volt + ((size_t)t_hi * P.n_chan + c) * row_bytes + (P.n_pol == 2 ? t.n_ant : 0);
+      for (int q = tid; q < (t.n_ant >> 2); q += NT_A) {
+        const uint32_t wlo = t_lo < P.n_t ? __ldg(reinterpret_cast<const uint32_t*>(lo) + q) : 0u;
+        const uint32_t whi = t_hi < P.n_t ? __ldg(reinterpret_cast<const uint32_t*>(hi) + q) : 0u;
+        unpack_words(wlo, whi, E + 4 * q, tid >> 1);
+      }
+      // the barrier after the zero fill below publishes E (the previous item's gather is behind
+      // that item's barriers)
+    }
     const int y0 = g * RG, rows = min(RG, t.R - y0);
     for (int i = tid; i < RG * N; i += NT_A) buf[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     __syncthreads();
@@ -108,15 +116,28 @@ __global__ void __launch_bounds__(NT_A) tiled_rows(TiledParams P) {
     for (uint32_t ci = cbeg + tid; ci < cend; ci += NT_A) {
       const CellRec cell = t.cells[ci];
       float2 sr = make_float2(0.0f, 0.0f), si = make_float2(0.0f, 0.0f);
-      for (uint32_t e = cell.ent_begin; e < cell.ent_begin + cell.ent_count; ++e) {
-        const float4 v = E[__ldg(t.ent_ant + e)];
-        const float2 vr = make_float2(v.x, v.y), vi = make_float2(v.z, v.w);
-        if (DELTA) {
-          sr = __fadd2_rn(sr, vr); si = __fadd2_rn(si, vi);
-        } else {
-          const float2 w = __ldg(t.ent_tap + e);
-          sr = __ffma2_rn(vr, f2(w.x), sr); sr = __ffma2_rn(neg2(vi), f2(w.y), sr);
-          si = __ffma2_rn(vi, f2(w.x), si); si = __ffma2_rn(vr, f2(w.y), si);
+      const uint32_t e_end = cell.ent_begin + cell.ent_count;
+      for (uint32_t e = cell.ent_begin; e < e_end; e += 4) {  // table loads of 4 entries in flight
+        uint32_t an[4];
+        float2 wt[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const uint32_t ee = min(e + k, e_end - 1);
+          an[k] = __ldg(t.ent_ant + ee);
+          if (!DELTA) wt[k] = __ldg(t.ent_tap + ee);
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          if (e + k < e_end) {
+            const float4 v = E[an[k]];
+            const float2 vr = make_float2(v.x, v.y), vi = make_float2(v.z, v.w);
+            if (DELTA) {
+              sr = __fadd2_rn(sr, vr); si = __fadd2_rn(si, vi);
+            } else {
+              sr = __ffma2_rn(vr, f2(wt[k].x), sr); sr = __ffma2_rn(neg2(vi), f2(wt[k].y), sr);
+              si = __ffma2_rn(vi, f2(wt[k].x), si); si = __ffma2_rn(vr, f2(wt[k].y), si);
+            }
+          }
         }
       }
       buf[(cell.y - y0) * N + cell.x] = make_float4(sr.x, sr.y, si.x, si.y);
@@ -200,7 +221,7 @@ __device__ __forceinline__ void accumulate_products(const C2& z, float2& acc, fl
 
 template <int J, int NPROD>
 __global__ void __launch_bounds__(NT_B) tiled_cols(TiledParams P) {
-  constexpr int N = 32 * J, M = 16 * J, W = 64 / J, XS = x_team_stride<J>();
+  constexpr int N = 32 * J, M = 16 * J, W = 64 / J, XS = x_team_stride_cols<J>();
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const DevTables& t = P.t;
   const int R = t.R;
@@ -323,7 +344,7 @@ size_t rows_smem_bytes(int n_ant) {
 }
 template <int J>
 size_t cols_smem_bytes(int R) {
-  constexpr int W = 64 / J, XS = x_team_stride<J>();
+  constexpr int W = 64 / J, XS = x_team_stride_cols<J>();
   return ((size_t)2 * W * XS + 2 * TWV + 2 * 16 * TWV + (size_t)2 * (R + 1) * W) * sizeof(float4);
 }
 
@@ -342,6 +363,14 @@ int launch_cols(const TiledParams& P, dim3 grid, size_t smem, cudaStream_t s) {
   return EPIC_OK;
 }
 
+template <int J, int NPROD>
+int cols_occupancy(int* occ, size_t smem) {
+  int st = set_dyn_smem(tiled_cols<J, NPROD>, smem);
+  if (st != EPIC_OK) return st;
+  EPIC_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, tiled_cols<J, NPROD>, NT_B, smem));
+  return EPIC_OK;
+}
+
 template <int J>
 int tiled_image_j(epic_plan* p, const ImageArgs& a, TiledParams& P) {
   constexpr int N = 32 * J, W = 64 / J, RG = NT_A / (2 * J);
@@ -350,15 +379,23 @@ int tiled_image_j(epic_plan* p, const ImageArgs& a, TiledParams& P) {
   const size_t frame_bytes = (size_t)R * N * sizeof(float4);
   const long long max_frames = (long long)std::max<size_t>(1, p->scratch_bytes / frame_bytes);
   const int strips = N / W;
-  // kernel B wants ~3 CTAs per SM: strips x Cb of them; the rest of the scratch goes to time
-  long long Cb = std::min<long long>(a.n_chan, (3LL * p->n_sm + strips - 1) / strips);
-  Cb = std::max<long long>(1, std::min(Cb, max_frames));
-  const long long Tb = std::max<long long>(1, std::min<long long>(n_pairs, max_frames / Cb));
-  const int n_groups = (R + RG - 1) / RG;
   const size_t smem_a = rows_smem_bytes<J>(p->n_ant), smem_b = cols_smem_bytes<J>(R);
   const bool delta = p->t.is_delta != 0;
   int st = delta ? set_dyn_smem(tiled_rows<J, true>, smem_a) : set_dyn_smem(tiled_rows<J, false>, smem_a);
   if (st != EPIC_OK) return st;
+  // both kernels run as ONE wave: strips x Cb column CTAs, and an equal share of the row items per CTA
+  int occ_a = 0, occ_b = 0;
+  if (delta) EPIC_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_a, tiled_rows<J, true>, NT_A, smem_a));
+  else EPIC_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_a, tiled_rows<J, false>, NT_A, smem_a));
+  if (a.n_products == 1) st = cols_occupancy<J, 1>(&occ_b, smem_b);
+  else if (a.n_products == 2) st = cols_occupancy<J, 2>(&occ_b, smem_b);
+  else st = cols_occupancy<J, 4>(&occ_b, smem_b);
+  if (st != EPIC_OK) return st;
+  if (occ_a < 1 || occ_b < 1) return EPIC_ERR_RANGE;
+  long long Cb = std::min<long long>(a.n_chan, ((long long)occ_b * p->n_sm) / strips);
+  Cb = std::max<long long>(1, std::min(Cb, max_frames));
+  const long long Tb = std::max<long long>(1, std::min<long long>(n_pairs, max_frames / Cb));
+  const int n_groups = (R + RG - 1) / RG;
   int launches = 0;
   for (int c0 = 0; c0 < a.n_chan; c0 += (int)Cb) {
     P.c0 = c0;
@@ -366,9 +403,8 @@ int tiled_image_j(epic_plan* p, const ImageArgs& a, TiledParams& P) {
     for (int p0 = 0; p0 < n_pairs; p0 += (int)Tb) {
       P.p0 = p0;
       P.Tb = (int)std::min<long long>(Tb, n_pairs - p0);
-      const int frames = P.Cb * P.Tb;
-      const int split = std::max(1, std::min(n_groups, (2 * p->n_sm + frames - 1) / frames));
-      const dim3 grid_a(frames, split);
+      const long long items = (long long)P.Cb * P.Tb * n_groups;
+      const dim3 grid_a((unsigned)std::min<long long>(items, (long long)occ_a * p->n_sm));
       if (delta) tiled_rows<J, true><<<grid_a, NT_A, smem_a, a.stream>>>(P);
       else tiled_rows<J, false><<<grid_a, NT_A, smem_a, a.stream>>>(P);
       const dim3 grid_b(strips, P.Cb);
