@@ -274,7 +274,7 @@ def run_epic(args, wl):
             "peak_measured_fma_probe": probe["tflops"], "frac_of_measured_probe": achieved / probe["tflops"],
             "algorithmic_flops_per_frame": flops, "algorithmic_bytes_per_frame": bytes_f,
             "hbm_achieved_gbs": bytes_f * wl.frames / (kernel_ms * 1e-3) / 1e9,
-            "kernel_ms": kernel_ms, "kernel": "epic_fused" if path == 2 else "grid_rowfft+colfft_accum",
+            "kernel_ms": kernel_ms, "kernel": PATH_KERNELS.get(path, str(path)),
         },
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(volt.nbytes),
                 "d2h_bytes_per_step": int(out.numel() * 4)},

@@ -26,7 +26,7 @@
 // complex numbers read from shared memory; see TwSet).  Rows (along x, rho = l2) and columns
 // (along y, rho = m2) run the SAME code, so the hot loop is a few KB of instructions shared by
 // all warps.  (The first version of this kernel unrolled every residue with immediate twiddles:
-// 109 KB of code, instruction-fetch bound at 0.36 of the roofline; profiles/r01_fused_history.md.)
+// 109 KB of code, instruction-fetch bound at 0.36 of the roofline; profiles/r01_fused_c2_ncu.md.)
 //
 //   per batch of F pairs (F time samples when n_pol == 2):
 //     prefetch  next batch's 4+4-bit voltages, global -> registers (consumed one batch later)
