@@ -54,7 +54,7 @@ typedef enum epic_status {
 typedef enum epic_path {
   EPIC_PATH_AUTO = 0,
   EPIC_PATH_TWOPASS = 1, /* grid+row-FFT kernel -> L2-resident scratch -> column-FFT+products kernel */
-  EPIC_PATH_FUSED = 2,   /* one kernel, planes never leave the SM (occupied cells within 32x32, N = 64, 128) */
+  EPIC_PATH_FUSED = 2,   /* one kernel (+ a tiny ordered fix-up of split units), planes never leave the SM (occupied cells within 32x32, N = 64, 128) */
   EPIC_PATH_TILED = 3    /* N = 256, 512: packed row kernel -> L2-resident scratch -> packed column kernel */
 } epic_path;
 

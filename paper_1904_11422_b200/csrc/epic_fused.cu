@@ -35,7 +35,8 @@
 //     rows      S4 along x, thread = (pair, row y, h), in place
 //     unpack    S1: the prefetched words -> E (float4 per antenna) for the NEXT batch
 //     columns   S4 along y + S5 + S6: thread = (l1, rho'); 16 outputs -> products -> += registers
-//   at the end of the unit's time range: one add per pixel into out_accum.
+//   at the end of the unit's time range: one add per pixel into out_accum (directly, or through
+//   the partial-sum fix-up kernel when the unit's time range was split between two CTAs).
 #include <algorithm>
 
 #include "epic_internal.h"
@@ -92,6 +93,7 @@ struct FusedParams {
   const uint16_t* ent_ant;   // gather entries, sorted by block cell
   const float2* ent_tap;
   const float4* tw;          // [2Q][TWV]: the TwSet of every residue rho
+  float* partial;            // scratch [grid][2 slots][NACC][16][NT]: partial sums of split units
   int n_t, n_chan, n_ant, n_pol, n_planes;
   int R, Cc;                 // occupied rows / columns of the block
   int nb;                    // batches per unit
@@ -216,10 +218,51 @@ __device__ __forceinline__ void col_task(const float4* __restrict__ col, const f
   }
 }
 
+// out_accum planes of one pixel += v (reading Q14: {XX} | {XX,YY} | {XX,YY,Re XY,Im XY,Re YX,Im YX})
+template <int NPROD>
+__device__ __forceinline__ void add_pixel(float* __restrict__ px, size_t plane, const float* v) {
+  px[0] += v[0];
+  if constexpr (NPROD >= 2) px[plane] += v[1];
+  if constexpr (NPROD == 4) {  // YX = conj(XY)
+    px[2 * plane] += v[2];
+    px[3 * plane] += v[3];
+    px[4 * plane] += v[2];
+    px[5 * plane] -= v[3];
+  }
+}
+
+// Adds the parked partial sums of every unit whose time range was split between CTAs, in CTA
+// order.  One CTA per unit, same thread <-> pixel mapping as the main kernel.
+template <int Q, int NPROD>
+__global__ void __launch_bounds__(64 * Q) epic_fused_fixup(FusedParams P, int main_grid) {
+  constexpr int NT = 64 * Q, N = 32 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
+  const int unit = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const long long G = main_grid, first = (long long)unit * P.nb, last = first + P.nb - 1;
+  const int b_lo = (int)(((first + 1) * G - 1) / P.total), b_hi = (int)(((last + 1) * G - 1) / P.total);
+  if (b_lo == b_hi) return;  // the unit ran in one CTA and was added directly
+  const int l1 = (warp & 1) * 16 + (lane >> 1);
+  const int rho = (warp >> 1) * 2 + (lane & 1);
+  const int c = unit / Q, l2 = unit - c * Q;
+  const size_t plane = (size_t)N * N;
+  float* o = P.out + (size_t)c * P.n_planes * plane + (Q * l1 + l2);
+  for (int k = 0; k < 16; ++k) {
+    float v[NACC];
+#pragma unroll
+    for (int q = 0; q < NACC; ++q) v[q] = 0.0f;
+    for (int b = b_lo; b <= b_hi; ++b) {
+      const int slot = (first <= P.total * b / G) ? 0 : 1;  // does the segment start the CTA's range?
+      const float* part = P.partial + ((size_t)(b * 2 + slot) * NACC * 16) * NT + tid;
+#pragma unroll
+      for (int q = 0; q < NACC; ++q) v[q] += part[(size_t)(q * 16 + k) * NT];
+    }
+    add_pixel<NPROD>(o + (size_t)(2 * Q * k + rho) * N, plane, v);
+  }
+}
+
 template <int Q, int NPROD, bool DELTA, int NB>
 __global__ void __launch_bounds__(64 * Q, NPROD == 4 ? 1 : 2)
 epic_fused_kernel(FusedParams P) {
-  constexpr int NT = 64 * Q, N = 32 * Q;
+  constexpr int NT = 64 * Q, N = 32 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* gh = reinterpret_cast<float4*>(smem_raw);  // [F][32][HS]
   float4* tws = gh + F * PLANE;                      // [2Q][TWV]
@@ -251,32 +294,39 @@ epic_fused_kernel(FusedParams P) {
 #pragma unroll
   for (int k = 0; k < (NPROD == 4 ? 16 : 1); ++k) xy[k] = make_float2(0.0f, 0.0f);
 
-  auto flush = [&](int unit) {
+  // S6.  A unit whose whole time range ran in this CTA is added to out_accum directly (this CTA
+  // is the only writer of those pixels).  When the equal split of the work list cut a unit's time
+  // range between CTAs, each CTA parks its partial sums in the scratch (slot 0: the segment that
+  // starts the CTA's range, slot 1: the one that ends it) and epic_fused_fixup adds them in CTA
+  // order: no atomics anywhere, and the result does not depend on scheduling.
+  auto flush = [&](int unit, bool complete, int slot) {
     const int c = unit / Q, l2 = unit - c * Q;
     const size_t plane = (size_t)N * N;
     float* o = P.out + (size_t)c * P.n_planes * plane + (Q * l1 + l2);
+    float* part = P.partial + ((size_t)(blockIdx.x * 2 + slot) * NACC * 16) * NT + tid;
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
-      float* px = o + (size_t)(2 * Q * k + rho) * N;
+      float v[NACC];
       if constexpr (NPROD == 1) {
-        atomicAdd(px, acc[k].x + acc[k].y);
+        v[0] = acc[k].x + acc[k].y;
       } else {
-        atomicAdd(px, acc[k].x);
-        atomicAdd(px + plane, acc[k].y);
+        v[0] = acc[k].x; v[1] = acc[k].y;
       }
-      if constexpr (NPROD == 4) {  // YX = conj(XY)
-        atomicAdd(px + 2 * plane, xy[k].x);
-        atomicAdd(px + 3 * plane, xy[k].y);
-        atomicAdd(px + 4 * plane, xy[k].x);
-        atomicAdd(px + 5 * plane, -xy[k].y);
-        xy[k] = make_float2(0.0f, 0.0f);
-      }
+      if constexpr (NPROD == 4) { v[2] = xy[k].x; v[3] = xy[k].y; xy[k] = make_float2(0.0f, 0.0f); }
       acc[k] = make_float2(0.0f, 0.0f);
+      if (complete) {
+        add_pixel<NPROD>(o + (size_t)(2 * Q * k + rho) * N, plane, v);
+      } else {
+#pragma unroll
+        for (int q = 0; q < NACC; ++q) part[(size_t)(q * 16 + k) * NT] = v[q];
+      }
     }
   };
 
   int unit = (int)(g0 / P.nb);
   int b = (int)(g0 - (long long)unit * P.nb);
+  const int first_unit = unit;
+  int seg_begin = b;  // first batch of the current unit done by this CTA
   PrefetchSlots ps;
   prefetch_init<NT>(P, tid, ps);
   uint32_t wlo[MAXW], whi[MAXW];
@@ -314,7 +364,10 @@ epic_fused_kernel(FusedParams P) {
       col_task<NB, NPROD>(gh + f * PLANE + l1, tws + tw_off, acc, xy);
     }
 
-    if (unit_n != unit || !more) flush(unit);
+    if (unit_n != unit || !more) {
+      flush(unit, seg_begin == 0 && b == P.nb - 1, unit == first_unit ? 0 : 1);
+      seg_begin = 0;
+    }
     unit = unit_n; b = b_n;
     __syncthreads();  // next batch's E is complete; gh is free
   }
@@ -342,7 +395,10 @@ int launch_fused(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
   if (per_sm < 1) return EPIC_ERR_RANGE;
   const long long slots = (long long)per_sm * p->n_sm;
   const int grid = (int)std::min<long long>(P.total, slots);
+  constexpr int NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
+  if ((size_t)grid * 2 * NACC * 16 * NT * sizeof(float) > p->scratch_bytes) return EPIC_ERR_RANGE;
   kern<<<grid, NT, smem, s>>>(P);
+  epic_fused_fixup<Q, NPROD><<<(unsigned)(P.total / P.nb), NT, 0, s>>>(P, grid);
   EPIC_CUDA_TRY(cudaGetLastError());
   return EPIC_OK;
 }
@@ -462,6 +518,7 @@ int fused_image(epic_plan* p, const ImageArgs& a) {
   P.ent_ant = p->t.ent_ant;
   P.ent_tap = p->t.ent_tap;
   P.tw = ft->tw;
+  P.partial = static_cast<float*>(p->d_scratch);
   P.n_t = a.n_t;
   P.n_chan = a.n_chan;
   P.n_ant = p->n_ant;
@@ -476,7 +533,7 @@ int fused_image(epic_plan* p, const ImageArgs& a) {
   if (Q == 2) st = launch_fused_q<2>(p, P, a.n_products, a.stream);
   else st = launch_fused_q<4>(p, P, a.n_products, a.stream);
   if (st != EPIC_OK) return st;
-  p->last_launches = 1;
+  p->last_launches = 2;  // the fused kernel and the (tiny) fix-up of split units
   return EPIC_OK;
 }
 
