@@ -23,6 +23,7 @@
 // twiddles (epic_packed.cuh), which come from plan tables computed in double.
 #include <algorithm>
 #include <cmath>
+#include <cstring>
 #include <new>
 #include <vector>
 
@@ -49,6 +50,7 @@ struct TiledParams {
   float* out;            // [C][planes][N][N]
   const float4* tw1;     // [2][TWV]      step-1 TwSet of rho (base r^J)
   const float4* tw2;     // [2][16][TWV]  step-2 twiddles of (rho, k1) (base r W_M^{k1})
+  const float4* ent_rec; // [n_ent] gather entries as one 16-byte record: (tap.re, tap.im, antenna index bits, 0)
   int n_t, n_chan, n_pol, n_planes;
   int c0, p0, Cb, Tb;    // batch: channels [c0, c0+Cb) x pairs [p0, p0+Tb)
   int nbx, nby;          // prefold counts along x (row pass) and y (column pass)
@@ -90,6 +92,7 @@ __global__ void __launch_bounds__(NT_A) tiled_rows(TiledParams P) {
   const long long n_items = (long long)P.Cb * P.Tb * n_groups;
   const int item0 = (int)(n_items * blockIdx.x / gridDim.x), item1 = (int)(n_items * (blockIdx.x + 1) / gridDim.x);
   int fb_loaded = -1;
+  for (int i = tid; i < RG * N; i += NT_A) buf[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
   for (int item = item0; item < item1; ++item) {
     const int fb = item / n_groups, g = item - fb * n_groups;
     if (fb != fb_loaded) {  // S1: this frame pair's voltages -> E
@@ -105,60 +108,57 @@ __global__ void __launch_bounds__(NT_A) tiled_rows(TiledParams P) {
         const uint32_t whi = t_hi < P.n_t ? __ldg(reinterpret_cast<const uint32_t*>(hi) + q) : 0u;
         unpack_words(wlo, whi, E + 4 * q, tid >> 1);
       }
-      // the barrier after the zero fill below publishes E (the previous item's gather is behind
-      // that item's barriers)
     }
+    __syncthreads();  // E and the zeroed row buffer (end of the previous item) are complete
     const int y0 = g * RG, rows = min(RG, t.R - y0);
-    for (int i = tid; i < RG * N; i += NT_A) buf[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-    __syncthreads();
-    // S3: gather-gridding of the group's cells, one thread per cell, sums in table order
+    // S3: gather-gridding of the group's cells, one thread per cell, sums in table order.
+    // Four cell records, then four entry records, are in flight per thread (L2 latency).
     const uint32_t cbeg = __ldg(t.row_ptr + y0), cend = __ldg(t.row_ptr + y0 + rows);
-    for (uint32_t ci = cbeg + tid; ci < cend; ci += NT_A) {
-      const CellRec cell = t.cells[ci];
-      float2 sr = make_float2(0.0f, 0.0f), si = make_float2(0.0f, 0.0f);
-      const uint32_t e_end = cell.ent_begin + cell.ent_count;
-      for (uint32_t e = cell.ent_begin; e < e_end; e += 4) {  // table loads of 4 entries in flight
-        uint32_t an[4];
-        float2 wt[4];
+    for (uint32_t base = cbeg + tid; base < cend; base += 4 * NT_A) {
+      CellRec cr[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          const uint32_t ee = min(e + k, e_end - 1);
-          an[k] = __ldg(t.ent_ant + ee);
-          if (!DELTA) wt[k] = __ldg(t.ent_tap + ee);
-        }
+      for (int q = 0; q < 4; ++q) cr[q] = t.cells[min(base + q * NT_A, cend - 1)];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          if (e + k < e_end) {
-            const float4 v = E[an[k]];
-            const float2 vr = make_float2(v.x, v.y), vi = make_float2(v.z, v.w);
-            if (DELTA) {
-              sr = __fadd2_rn(sr, vr); si = __fadd2_rn(si, vi);
-            } else {
-              sr = __ffma2_rn(vr, f2(wt[k].x), sr); sr = __ffma2_rn(neg2(vi), f2(wt[k].y), sr);
-              si = __ffma2_rn(vi, f2(wt[k].x), si); si = __ffma2_rn(vr, f2(wt[k].y), si);
+      for (int q = 0; q < 4; ++q) {
+        if (base + q * NT_A >= cend) break;
+        const CellRec cell = cr[q];
+        float2 sr = make_float2(0.0f, 0.0f), si = make_float2(0.0f, 0.0f);
+        const uint32_t e_end = cell.ent_begin + cell.ent_count;
+        for (uint32_t e = cell.ent_begin; e < e_end; e += 4) {
+          float4 rec[4];  // (tap.re, tap.im, antenna, -)
+#pragma unroll
+          for (int k = 0; k < 4; ++k) rec[k] = __ldg(P.ent_rec + min(e + k, e_end - 1));
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            if (e + k < e_end) {
+              const float4 v = E[__float_as_uint(rec[k].z)];
+              const float2 vr = make_float2(v.x, v.y), vi = make_float2(v.z, v.w);
+              if (DELTA) {
+                sr = __fadd2_rn(sr, vr); si = __fadd2_rn(si, vi);
+              } else {
+                sr = __ffma2_rn(vr, f2(rec[k].x), sr); sr = __ffma2_rn(neg2(vi), f2(rec[k].y), sr);
+                si = __ffma2_rn(vi, f2(rec[k].x), si); si = __ffma2_rn(vr, f2(rec[k].y), si);
+              }
             }
           }
         }
+        buf[(cell.y - y0) * N + cell.x] = make_float4(sr.x, sr.y, si.x, si.y);
       }
-      buf[(cell.y - y0) * N + cell.x] = make_float4(sr.x, sr.y, si.x, si.y);
     }
     __syncthreads();
-    if (P.nbx > 0) {  // prefold: (a, b) <- (a + b, a - b) for the few x that have a partner x + M
-      for (int i = tid; i < RG * P.nbx; i += NT_A) {
-        const int rr = i / P.nbx, x = i - rr * P.nbx;
-        const C2 a = to_c2(buf[rr * N + x]), b = to_c2(buf[rr * N + x + M]);
-        buf[rr * N + x] = make_float4(a.re.x + b.re.x, a.re.y + b.re.y, a.im.x + b.im.x, a.im.y + b.im.y);
-        buf[rr * N + x + M] = make_float4(a.re.x - b.re.x, a.re.y - b.re.y, a.im.x - b.im.x, a.im.y - b.im.y);
-      }
-      __syncthreads();
-    }
     C2 z[16];
-    {  // step 1: 16-point ramped FFT of s_rho[J i + j]
+    {  // step 1 inputs: s_rho[J i + j] = in[x] +- in[x + M] for the nbx elements that have a partner
       const float4* row = buf + r * N;
 #pragma unroll
       for (int i = 0; i < 16; ++i) {
         const int x = J * i + j;
-        z[bitrev4t(i)] = to_c2(row[(rho && x < P.nbx) ? x + M : x]);
+        C2 a = to_c2(row[x]);
+        if (x < P.nbx) {
+          const C2 b = to_c2(row[x + M]);
+          const float2 sg = f2(rho ? -1.0f : 1.0f);
+          a.re = __ffma2_rn(b.re, sg, a.re); a.im = __ffma2_rn(b.im, sg, a.im);
+        }
+        z[bitrev4t(i)] = a;
       }
     }
     __syncthreads();  // every thread holds its inputs: buf becomes the exchange buffer
@@ -170,37 +170,39 @@ __global__ void __launch_bounds__(NT_A) tiled_rows(TiledParams P) {
       for (int k1 = 0; k1 < 16; ++k1) xt[j * XJ + k1] = to_f4(z[k1]);
     }
     __syncthreads();
-    // step 2: thread t = j takes k1 = t (and t + 8 when J == 8)
+    // step 2: thread t = j takes k1 = t (and t + 8 when J == 8); outputs l = 2 (k1 + 16 k2) + rho go
+    // straight to H: for one k2 the 2 J lanes of a team write 2 J consecutive float4
+    float4* hrow = P.H + ((size_t)fb * t.R + y0 + r) * N + rho;
     if constexpr (J == 8) {
       C2 za[8], zb[8];
 #pragma unroll
       for (int q = 0; q < 8; ++q) { za[bitrev3(q)] = to_c2(xt[q * XJ + j]); zb[bitrev3(q)] = to_c2(xt[q * XJ + j + 8]); }
-      __syncthreads();  // exchange buffer consumed: buf becomes the output rows
+      __syncthreads();  // exchange buffer consumed: the row buffer is zeroed for the next item
+      for (int i = tid; i < RG * N; i += NT_A) buf[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
       const float4 *ta = tw2 + (rho * 16 + j) * TWV, *tb = tw2 + (rho * 16 + j + 8) * TWV;
       const float4 a0 = ta[0], a1 = ta[1], b0 = tb[0], b1 = tb[1];
       fft8_ramped(za, a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w);
       fft8_ramped(zb, b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w);
-      float4* row = buf + r * N + rho;
+      if (r < rows) {
 #pragma unroll
-      for (int k2 = 0; k2 < 8; ++k2) {
-        row[2 * (j + 16 * k2)] = to_f4(za[k2]);
-        row[2 * (j + 8 + 16 * k2)] = to_f4(zb[k2]);
+        for (int k2 = 0; k2 < 8; ++k2) {
+          hrow[2 * (j + 16 * k2)] = to_f4(za[k2]);
+          hrow[2 * (j + 8 + 16 * k2)] = to_f4(zb[k2]);
+        }
       }
     } else {
 #pragma unroll
       for (int q = 0; q < 16; ++q) z[bitrev4t(q)] = to_c2(xt[q * XJ + j]);
       __syncthreads();
+      for (int i = tid; i < RG * N; i += NT_A) buf[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
       const float4* tw = tw2 + (rho * 16 + j) * TWV;
       const float4 t0 = tw[0];
       fft16_ramped(z, tw, t0.z, t0.w);
-      float4* row = buf + r * N + rho;
+      if (r < rows) {
 #pragma unroll
-      for (int k2 = 0; k2 < 16; ++k2) row[2 * (j + 16 * k2)] = to_f4(z[k2]);
+        for (int k2 = 0; k2 < 16; ++k2) hrow[2 * (j + 16 * k2)] = to_f4(z[k2]);
+      }
     }
-    __syncthreads();
-    float4* dst = P.H + ((size_t)fb * t.R + y0) * N;
-    for (int i = tid; i < rows * N; i += NT_A) dst[i] = buf[i];
-    __syncthreads();
   }
 }
 
@@ -261,22 +263,19 @@ __global__ void __launch_bounds__(NT_B) tiled_cols(TiledParams P) {
     cp_async_wait_all();
     __syncthreads();  // this frame's tile is complete; the previous frame is done with xbuf and the other tile
     if (pb + 1 < P.Tb) stage(pb + 1, (pb + 1) & 1);
-    if (P.nby > 0) {  // prefold along y
-      for (int i = tid; i < P.nby * W; i += NT_B) {
-        const C2 a = to_c2(cur[i]), b = to_c2(cur[i + M * W]);
-        cur[i] = make_float4(a.re.x + b.re.x, a.re.y + b.re.y, a.im.x + b.im.x, a.im.y + b.im.y);
-        cur[i + M * W] = make_float4(a.re.x - b.re.x, a.re.y - b.re.y, a.im.x - b.im.x, a.im.y - b.im.y);
-      }
-      __syncthreads();
-    }
     {  // step 1
       C2 z[16];
 #pragma unroll
       for (int i = 0; i < 16; ++i) {
         const int y = J * i + j;
-        int ys = (rho && y < P.nby) ? y + M : y;
-        ys = ys < R ? ys : R;  // rows beyond the occupied box: the zero row
-        z[bitrev4t(i)] = to_c2(cur[ys * W + w]);
+        const int ys = y < R ? y : R;  // rows beyond the occupied box: the zero row
+        C2 a = to_c2(cur[ys * W + w]);
+        if (y < P.nby) {  // the few rows that have a partner y + M (prefold)
+          const C2 b = to_c2(cur[(y + M) * W + w]);
+          const float2 sg = f2(rho ? -1.0f : 1.0f);
+          a.re = __ffma2_rn(b.re, sg, a.re); a.im = __ffma2_rn(b.im, sg, a.im);
+        }
+        z[bitrev4t(i)] = a;
       }
       const float4* tw = tw1 + rho * TWV;
       const float4 t0 = tw[0];
@@ -334,6 +333,7 @@ __global__ void __launch_bounds__(NT_B) tiled_cols(TiledParams P) {
 struct TiledTables {
   float4* tw1;
   float4* tw2;
+  float4* ent_rec;
 };
 
 template <int J>
@@ -458,8 +458,17 @@ int tiled_plan_init(epic_plan* p) {
   }
   TiledTables* tt = new (std::nothrow) TiledTables();
   if (!tt) return EPIC_ERR_NOMEM;
-  tt->tw1 = tt->tw2 = nullptr;
+  std::vector<float4> rec(std::max<size_t>(1, p->h_ent_ant.size()));
+  for (size_t e = 0; e < p->h_ent_ant.size(); ++e) {
+    const uint32_t ant = p->h_ent_ant[e];
+    float antf;
+    std::memcpy(&antf, &ant, sizeof(float));
+    rec[e] = make_float4(p->h_ent_tap[e].x, p->h_ent_tap[e].y, antf, 0.0f);
+  }
+  tt->tw1 = tt->tw2 = tt->ent_rec = nullptr;
   cudaError_t ce = cudaMalloc(&tt->tw1, tw1.size() * sizeof(float4));
+  if (ce == cudaSuccess) ce = cudaMalloc(&tt->ent_rec, rec.size() * sizeof(float4));
+  if (ce == cudaSuccess) ce = cudaMemcpy(tt->ent_rec, rec.data(), rec.size() * sizeof(float4), cudaMemcpyHostToDevice);
   if (ce == cudaSuccess) ce = cudaMalloc(&tt->tw2, tw2.size() * sizeof(float4));
   if (ce == cudaSuccess) ce = cudaMemcpy(tt->tw1, tw1.data(), tw1.size() * sizeof(float4), cudaMemcpyHostToDevice);
   if (ce == cudaSuccess) ce = cudaMemcpy(tt->tw2, tw2.data(), tw2.size() * sizeof(float4), cudaMemcpyHostToDevice);
@@ -467,6 +476,7 @@ int tiled_plan_init(epic_plan* p) {
     set_cuda_error(ce);
     if (tt->tw1) cudaFree(tt->tw1);
     if (tt->tw2) cudaFree(tt->tw2);
+    if (tt->ent_rec) cudaFree(tt->ent_rec);
     delete tt;
     return ce == cudaErrorMemoryAllocation ? EPIC_ERR_NOMEM : EPIC_ERR_CUDA;
   }
@@ -480,6 +490,7 @@ void tiled_plan_free(epic_plan* p) {
   if (tt) {
     if (tt->tw1) cudaFree(tt->tw1);
     if (tt->tw2) cudaFree(tt->tw2);
+    if (tt->ent_rec) cudaFree(tt->ent_rec);
     delete tt;
   }
   p->d_tiled = nullptr;
@@ -504,6 +515,7 @@ int tiled_image(epic_plan* p, const ImageArgs& a) {
   P.out = a.out;
   P.tw1 = tt->tw1;
   P.tw2 = tt->tw2;
+  P.ent_rec = tt->ent_rec;
   P.n_t = a.n_t;
   P.n_chan = a.n_chan;
   P.n_pol = a.n_pol;
