@@ -182,6 +182,8 @@ def run_epic(args, wl):
     plan.set_products(wl.n_products)
     if args.path:
         plan.set_path({"auto": 0, "twopass": 1, "fused": 2, "tiled": 3}[args.path])
+    if args.scratch_mib:
+        plan.set_scratch_limit(args.scratch_mib << 20)
     planes = plan.n_planes(wl.n_pol)
     out = torch.zeros((wl.n_chan, planes, wl.N, wl.N), dtype=torch.float32, device=dev)
     h_out = torch.empty(out.shape, dtype=torch.float32).pin_memory()
@@ -301,6 +303,7 @@ def main():
     ap.add_argument("--n-ant", type=int, default=None)
     ap.add_argument("--cpu-channels", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--scratch-mib", type=int, default=0, help="cap the per-batch scratch (tiled / two-pass paths)")
     args = ap.parse_args()
     wl = make_config(args.config, n_chan=args.n_chan, n_t=args.n_t, n_ant=args.n_ant)
     if args.impl == "reference":

@@ -83,6 +83,12 @@ EPIC_API int epic_plan_set_products(epic_plan* plan, int n_products);
 /* Select the kernel family (testing / benchmarking).  EPIC_ERR_RANGE if the plan cannot use it. */
 EPIC_API int epic_plan_set_path(epic_plan* plan, int path);
 
+/* Tuning: bytes of the plan's scratch (the intermediate H of the tiled / two-pass paths) one batch may
+ * use; 0 = all of it (1 GiB for N >= 256, else 64 MiB).  A small limit (e.g. 64 MiB) keeps H resident in
+ * the 126 MB L2 at the price of more, shorter batches, each ending in one read-modify-write of its
+ * channels' out_accum.  A batch always holds at least one frame. */
+EPIC_API int epic_plan_set_scratch_limit(epic_plan* plan, long long bytes);
+
 /* S1..S6 for one gulp (one call = one gulp of n_t samples).
  *   voltages   DEVICE uint8[n_t][n_chan][n_pol][n_ant] — [Time, Channel, Polarisation, Antenna]
  *              order, 1 byte = 4+4-bit complex: high nibble real, low nibble

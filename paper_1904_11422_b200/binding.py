@@ -24,6 +24,7 @@ SYMBOLS = {
     "epic_plan_destroy": (_i, [_vp]),
     "epic_plan_set_products": (_i, [_vp, _i]),
     "epic_plan_set_path": (_i, [_vp, _i]),
+    "epic_plan_set_scratch_limit": (_i, [_vp, ctypes.c_longlong]),
     "epic_image": (_i, [_vp, _vp, _i, _i, _i, _vp, _vp]),
     "epic_image_cf32": (_i, [_vp, _vp, _i, _i, _i, _vp, _vp]),
     "epic_plan_get_n": (_i, [_vp]),
@@ -138,6 +139,9 @@ class Plan:
     # -- configuration / queries
     def set_products(self, n_products: int) -> None:
         _check(lib().epic_plan_set_products(self._h, n_products), "epic_plan_set_products")
+
+    def set_scratch_limit(self, n_bytes: int):
+        _check(lib().epic_plan_set_scratch_limit(self._h, int(n_bytes)), "epic_plan_set_scratch_limit")
 
     def set_path(self, path: int) -> None:
         _check(lib().epic_plan_set_path(self._h, path), "epic_plan_set_path")

@@ -40,6 +40,7 @@ struct epic_plan {
   void* d_blob;                // one allocation holding all tables
   void* d_scratch;             // two-pass intermediate H, L2-sized
   size_t scratch_bytes;
+  size_t scratch_limit;        // bytes of the scratch a batch may use (0 = all of it)
   void* d_fused;               // tables private to the fused path
   int fused_ok;                // support fits the fused kernel
   void* d_tiled;               // tables private to the tiled path
@@ -80,6 +81,11 @@ int tiled_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products);
 int tiled_image(epic_plan* p, const ImageArgs& a);
 
 void set_cuda_error(cudaError_t e);
+
+// bytes of the plan's scratch one batch may use
+inline size_t scratch_budget(const epic_plan* p) {
+  return (p->scratch_limit != 0 && p->scratch_limit < p->scratch_bytes) ? p->scratch_limit : p->scratch_bytes;
+}
 
 } // namespace epic
 

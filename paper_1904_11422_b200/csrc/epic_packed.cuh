@@ -108,5 +108,25 @@ __device__ __forceinline__ void unpack_words(uint32_t wlo, uint32_t whi, float4*
   }
 }
 
+// Compact form of the same unpack for large antenna counts: one 32-bit word per antenna holding
+// the four biased nibbles as bytes (re_lo+8, re_hi+8, im_lo+8, im_hi+8); converted at use.
+__device__ __forceinline__ uint4 unpack_words_b8(uint32_t wlo, uint32_t whi) {
+  const uint32_t rl = ((wlo >> 4) & 0x0F0F0F0Fu) ^ 0x08080808u, il = (wlo & 0x0F0F0F0Fu) ^ 0x08080808u;
+  const uint32_t rh = ((whi >> 4) & 0x0F0F0F0Fu) ^ 0x08080808u, ih = (whi & 0x0F0F0F0Fu) ^ 0x08080808u;
+  uint32_t o[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const uint32_t re = __byte_perm(rl, rh, 0x0040u + 0x11u * (uint32_t)i);  // bytes (rl_i, rh_i, -, -)
+    const uint32_t im = __byte_perm(il, ih, 0x0040u + 0x11u * (uint32_t)i);
+    o[i] = __byte_perm(re, im, 0x5410u);
+  }
+  return make_uint4(o[0], o[1], o[2], o[3]);
+}
+__device__ __forceinline__ void b8_to_pair(uint32_t w, float2& vr, float2& vi) {
+  const float2 bias = f2(-12582920.0f);
+  vr = __fadd2_rn(make_float2(biased_byte_to_float_bits(w, 0), biased_byte_to_float_bits(w, 1)), bias);
+  vi = __fadd2_rn(make_float2(biased_byte_to_float_bits(w, 2), biased_byte_to_float_bits(w, 3)), bias);
+}
+
 }  // namespace
 }  // namespace epic

@@ -23,6 +23,8 @@
 // twiddles (epic_packed.cuh), which come from plan tables computed in double.
 #include <algorithm>
 #include <cmath>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -80,7 +82,7 @@ __global__ void __launch_bounds__(NT_A) tiled_rows(TiledParams P) {
   float4* buf = reinterpret_cast<float4*>(smem_raw);  // [BUF]
   float4* tw1 = buf + BUF;                            // [2][TWV]
   float4* tw2 = tw1 + 2 * TWV;                        // [2][16][TWV]
-  float4* E = tw2 + 2 * 16 * TWV;                     // [A]
+  uint32_t* E = reinterpret_cast<uint32_t*>(tw2 + 2 * 16 * TWV);  // [A] biased bytes (epic_packed.cuh)
   const int tid = threadIdx.x;
   const DevTables& t = P.t;
   for (int i = tid; i < 2 * TWV; i += NT_A) tw1[i] = __ldg(P.tw1 + i);
@@ -106,7 +108,7 @@ __global__ void __launch_bounds__(NT_A) tiled_rows(TiledParams P) {
       for (int q = tid; q < (t.n_ant >> 2); q += NT_A) {
         const uint32_t wlo = t_lo < P.n_t ? __ldg(reinterpret_cast<const uint32_t*>(lo) + q) : 0u;
         const uint32_t whi = t_hi < P.n_t ? __ldg(reinterpret_cast<const uint32_t*>(hi) + q) : 0u;
-        unpack_words(wlo, whi, E + 4 * q, tid >> 1);
+        *reinterpret_cast<uint4*>(E + 4 * q) = unpack_words_b8(wlo, whi);
       }
     }
     __syncthreads();  // E and the zeroed row buffer (end of the previous item) are complete
@@ -131,8 +133,8 @@ __global__ void __launch_bounds__(NT_A) tiled_rows(TiledParams P) {
 #pragma unroll
           for (int k = 0; k < 4; ++k) {
             if (e + k < e_end) {
-              const float4 v = E[__float_as_uint(rec[k].z)];
-              const float2 vr = make_float2(v.x, v.y), vi = make_float2(v.z, v.w);
+              float2 vr, vi;
+              b8_to_pair(E[__float_as_uint(rec[k].z)], vr, vi);
               if (DELTA) {
                 sr = __fadd2_rn(sr, vr); si = __fadd2_rn(si, vi);
               } else {
@@ -222,7 +224,7 @@ __device__ __forceinline__ void accumulate_products(const C2& z, float2& acc, fl
 }
 
 template <int J, int NPROD>
-__global__ void __launch_bounds__(NT_B) tiled_cols(TiledParams P) {
+__global__ void __launch_bounds__(NT_B, 3) tiled_cols(TiledParams P) {
   constexpr int N = 32 * J, M = 16 * J, W = 64 / J, XS = x_team_stride_cols<J>();
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const DevTables& t = P.t;
@@ -340,7 +342,7 @@ template <int J>
 size_t rows_smem_bytes(int n_ant) {
   constexpr int N = 32 * J, RG = NT_A / (2 * J), XS = x_team_stride<J>();
   constexpr int BUF = (RG * N > 2 * RG * XS) ? RG * N : 2 * RG * XS;
-  return ((size_t)BUF + 2 * TWV + 2 * 16 * TWV + (size_t)n_ant) * sizeof(float4);
+  return ((size_t)BUF + 2 * TWV + 2 * 16 * TWV) * sizeof(float4) + (size_t)n_ant * sizeof(uint32_t);
 }
 template <int J>
 size_t cols_smem_bytes(int R) {
@@ -377,7 +379,7 @@ int tiled_image_j(epic_plan* p, const ImageArgs& a, TiledParams& P) {
   const int R = p->R;
   const int n_pairs = a.n_pol == 2 ? a.n_t : (a.n_t + 1) / 2;
   const size_t frame_bytes = (size_t)R * N * sizeof(float4);
-  const long long max_frames = (long long)std::max<size_t>(1, p->scratch_bytes / frame_bytes);
+  const long long max_frames = (long long)std::max<size_t>(1, scratch_budget(p) / frame_bytes);
   const int strips = N / W;
   const size_t smem_a = rows_smem_bytes<J>(p->n_ant), smem_b = cols_smem_bytes<J>(R);
   const bool delta = p->t.is_delta != 0;
@@ -392,6 +394,7 @@ int tiled_image_j(epic_plan* p, const ImageArgs& a, TiledParams& P) {
   else st = cols_occupancy<J, 4>(&occ_b, smem_b);
   if (st != EPIC_OK) return st;
   if (occ_a < 1 || occ_b < 1) return EPIC_ERR_RANGE;
+  if (getenv("EPIC_DEBUG")) fprintf(stderr, "tiled: occ_a %d occ_b %d smem_a %zu smem_b %zu max_frames %lld\n", occ_a, occ_b, smem_a, smem_b, max_frames);
   long long Cb = std::min<long long>(a.n_chan, ((long long)occ_b * p->n_sm) / strips);
   Cb = std::max<long long>(1, std::min(Cb, max_frames));
   const long long Tb = std::max<long long>(1, std::min<long long>(n_pairs, max_frames / Cb));

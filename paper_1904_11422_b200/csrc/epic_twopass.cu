@@ -233,7 +233,7 @@ int twopass_image(epic_plan* p, const ImageArgs& a) {
   g.W = std::max(1, std::min(N, 2048 / N));
   const int strips = N / g.W;
   const size_t frame_bytes = (size_t)a.n_pol * R * N * sizeof(float2);
-  const long long max_frames = (long long)std::max<size_t>(1, p->scratch_bytes / frame_bytes);
+  const long long max_frames = (long long)std::max<size_t>(1, scratch_budget(p) / frame_bytes);
   const int want_blocks = 2 * p->n_sm;
   long long Cb = std::min<long long>(a.n_chan, (want_blocks + strips - 1) / strips);
   Cb = std::max<long long>(1, std::min(Cb, max_frames));

@@ -9,7 +9,7 @@ from oracle import epic_oracle as orc
 TOL = 1e-4  # BASELINE.json north_star: max |gpu - oracle| / image peak, fp32 path
 
 
-def run_gpu(wl, volt=None, path=None, calls=1, n_products=None, return_plan_info=False):
+def run_gpu(wl, volt=None, path=None, calls=1, n_products=None, return_plan_info=False, scratch_limit=None):
     import torch
     import paper_1904_11422_b200 as epic
 
@@ -19,6 +19,8 @@ def run_gpu(wl, volt=None, path=None, calls=1, n_products=None, return_plan_info
         plan.set_products(wl.n_products if n_products is None else n_products)
         if path is not None:
             plan.set_path(path)
+        if scratch_limit is not None:
+            plan.set_scratch_limit(scratch_limit)
         planes = plan.n_planes(wl.n_pol)
         out = torch.zeros((wl.n_chan, planes, wl.N, wl.N), dtype=torch.float32, device="cuda")
         dv = torch.from_numpy(v).cuda()

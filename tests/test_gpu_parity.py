@@ -185,8 +185,8 @@ def test_tiled_many_batches_accumulate():
     """More frames than one scratch batch holds, several channels: exercises the batch loop and
     the one-add-per-batch accumulation of the column kernel."""
     wl = make_config(4, n_chan=5, n_t=70)
-    gpu, info = run_gpu(wl, path=3, return_plan_info=True)
-    assert info["launches"] >= 4
+    gpu, info = run_gpu(wl, path=3, return_plan_info=True, scratch_limit=16 << 20)  # 31 frames per batch
+    assert info["launches"] >= 8
     ref = run_oracle(wl, channels=[0, 4])
     assert_parity(gpu[[0, 4]], ref, what="C4 5ch x 70")
 
