@@ -104,6 +104,16 @@ EPIC_API int epic_image(epic_plan* plan, const void* voltages, int n_t, int n_ch
 EPIC_API int epic_image_cf32(epic_plan* plan, const void* voltages_cf32, int n_t, int n_chan, int n_pol,
                     float* out_accum, epic_stream stream);
 
+/* Optional autocorrelation removal ("to remove the zero-spacing power inherent in EPIC";
+ * SURVEY.md 8(f) NEXT-2).  The EPIC image of a gulp is the direct-Fourier image of ALL antenna pairs,
+ * a = b included; this call SUBTRACTS from out_accum the a = b part of the same gulp,
+ *   sum_a (sum_t E_ap E_aq^*) |What_a[m][l]|^2,  What_a = transform of antenna a's gridded taps,
+ * for every product plane the plan forms (same arguments, layout and stream rules as epic_image; ci4
+ * voltages).  It is linear in the gulp, so it may be applied per call or to several gulps in turn.
+ * Four small kernels; reads the voltages once more; uses the plan's scratch. */
+EPIC_API int epic_autocorr_remove(epic_plan* plan, const void* voltages, int n_t, int n_chan, int n_pol,
+                         float* out_accum, epic_stream stream);
+
 /* Plan queries (host, synchronous). */
 EPIC_API int epic_plan_get_n(const epic_plan* plan);        /* N, or negative status */
 EPIC_API int epic_plan_get_n_planes(const epic_plan* plan, int n_pol); /* planes for current products */

@@ -32,7 +32,8 @@ test; S2 hand-worked cells incl. half-cells and wrap; S3 closed-form sums, colli
 linearity; S4 library inverse FFT vs the literal sum, impulse -> plane wave, zero-padding
 invariant; S5/S6 one- and two-antenna closed forms, YX = conj(XY); whole path: (a) FX
 equivalence with brute-force direct-Fourier imaging of all antenna pairs, (b) Parseval,
-(c) plane-wave source peaks at the predicted pixel with height A^2.
+(c) plane-wave source peaks at the predicted pixel with height A^2; autocorr_image:
+image minus it equals brute-force imaging of the pairs a != b, one antenna -> exactly the image.
 Parity unpinned: only the nibble-order *convention* (Q1) and anything LWA-instrument specific
 (no instrument data exists here); every function below has at least one pin.
 """
@@ -214,3 +215,40 @@ def epic_image(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Option
                 img[:, p] = xform(g)                         # S4
             acc[ci] += products(img, n_products).sum(axis=0)  # S5, S6
     return acc
+
+
+# ------------------------------------------------------------------ optional: autocorrelation removal
+def autocorr_image(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Optional[np.ndarray],
+                   grid_n: int, pad: int, n_products: int, kernel_k: int = 1,
+                   channels: Optional[list] = None) -> np.ndarray:
+    """The a = b part of the accumulated EPIC image ("the zero-spacing power inherent in
+    EPIC"), float64 [C'][planes][N][N], from the definition: the image is
+    sum_t A_p conj(A_q) with A_p = sum_a E_ap What_a, What_a = transform of antenna a gridded alone
+    with unit voltage; its a = b terms are  sum_a (sum_t E_ap conj(E_aq)) |What_a|^2.
+    Subtracting it from epic_image leaves the direct-Fourier image of the pairs a != b only
+    (pinned in tests/test_oracle_pins.py by brute force)."""
+    n = grid_n * pad
+    t_n, c_n, n_pol, n_ant = voltages.shape[:4]
+    ch = list(range(c_n)) if channels is None else list(channels)
+    cells = tap_cells(ant_uv, kernel_k, n)
+    w = taps_to_complex(taps, n_ant, kernel_k)
+    beam = np.empty((n_ant, n, n), dtype=np.float64)  # |What_a|^2
+    for a in range(n_ant):
+        one = np.zeros((1, n_ant), dtype=np.complex128)
+        one[0, a] = 1.0
+        beam[a] = np.abs(idft2_fast(grid_frames(one, cells, w, n))[0]) ** 2
+    pl = n_planes(n_pol, n_products)
+    out = np.zeros((len(ch), pl, n, n), dtype=np.float64)
+    for ci, c in enumerate(ch):
+        e = voltages_to_complex(voltages[:, c], kind)  # [T][Np][A]
+        vxx = (np.abs(e[:, 0]) ** 2).sum(axis=0)       # [A]
+        out[ci, 0] = np.tensordot(vxx, beam, axes=1)
+        if n_pol == 2:
+            vyy = (np.abs(e[:, 1]) ** 2).sum(axis=0)
+            out[ci, 1] = np.tensordot(vyy, beam, axes=1)
+            if n_products == 4:
+                vxy = (e[:, 0] * np.conj(e[:, 1])).sum(axis=0)
+                xy = np.tensordot(vxy, beam.astype(np.complex128), axes=1)
+                out[ci, 2], out[ci, 3] = xy.real, xy.imag
+                out[ci, 4], out[ci, 5] = xy.real, -xy.imag
+    return out

@@ -27,6 +27,7 @@ SYMBOLS = {
     "epic_plan_set_scratch_limit": (_i, [_vp, ctypes.c_longlong]),
     "epic_image": (_i, [_vp, _vp, _i, _i, _i, _vp, _vp]),
     "epic_image_cf32": (_i, [_vp, _vp, _i, _i, _i, _vp, _vp]),
+    "epic_autocorr_remove": (_i, [_vp, _vp, _i, _i, _i, _vp, _vp]),
     "epic_plan_get_n": (_i, [_vp]),
     "epic_plan_get_n_planes": (_i, [_vp, _i]),
     "epic_plan_get_cells": (_i, [_vp, _vp]),
@@ -177,6 +178,11 @@ class Plan:
         _check(lib().epic_image_cf32(self._h, _ptr(voltages), n_t, n_chan, n_pol, _ptr(out_accum),
                                      _stream(stream)), "epic_image_cf32")
 
+    def autocorr_remove(self, voltages, n_t: int, n_chan: int, n_pol: int, out_accum, stream=None) -> None:
+        """epic_autocorr_remove: subtract the a = b (zero-spacing) part of the same gulp."""
+        _check(lib().epic_autocorr_remove(self._h, _ptr(voltages), n_t, n_chan, n_pol, _ptr(out_accum),
+                                          _stream(stream)), "epic_autocorr_remove")
+
     def debug_grid(self, voltages, is_cf32: bool, n_pol: int, out_plane, stream=None) -> None:
         _check(lib().epic_debug_grid(self._h, _ptr(voltages), int(bool(is_cf32)), n_pol,
                                      _ptr(out_plane), _stream(stream)), "epic_debug_grid")
@@ -199,6 +205,10 @@ def epic_image(plan: Plan, voltages, n_t, n_chan, n_pol, out_accum, stream=None)
 
 def epic_image_cf32(plan: Plan, voltages, n_t, n_chan, n_pol, out_accum, stream=None) -> None:
     plan.image_cf32(voltages, n_t, n_chan, n_pol, out_accum, stream)
+
+
+def epic_autocorr_remove(plan: Plan, voltages, n_t, n_chan, n_pol, out_accum, stream=None) -> None:
+    plan.autocorr_remove(voltages, n_t, n_chan, n_pol, out_accum, stream)
 
 
 def epic_debug_unpack(bytes_dev, n: int, out_dev, stream=None) -> None:

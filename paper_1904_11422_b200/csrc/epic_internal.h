@@ -44,6 +44,7 @@ struct epic_plan {
   void* d_fused;               // tables private to the fused path
   int fused_ok;                // support fits the fused kernel
   void* d_tiled;               // tables private to the tiled path
+  void* d_auto;                // tap autocorrelation table of epic_autocorr_remove
   int tiled_ok;                // N is 256 or 512
   int n_sm;
   // host copies kept for the fused path's table builder
@@ -79,6 +80,11 @@ int tiled_plan_init(epic_plan* p);  // sets p->tiled_ok, allocates p->d_tiled
 void tiled_plan_free(epic_plan* p);
 int tiled_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products);
 int tiled_image(epic_plan* p, const ImageArgs& a);
+
+// epic_autocorr.cu
+int autocorr_plan_init(epic_plan* p, const float* taps);  // allocates p->d_auto
+void autocorr_plan_free(epic_plan* p);
+int autocorr_remove(epic_plan* p, const ImageArgs& a);
 
 void set_cuda_error(cudaError_t e);
 

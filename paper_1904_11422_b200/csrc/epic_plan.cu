@@ -242,6 +242,7 @@ int epic_plan_create(epic_plan** out, int grid_n, int pad, int n_ant, const floa
   p->fused_ok = 0;
   p->d_tiled = nullptr;
   p->tiled_ok = 0;
+  p->d_auto = nullptr;
   p->scratch_bytes = 0;
   p->scratch_limit = 0;
   int dev = 0;
@@ -275,6 +276,7 @@ int epic_plan_create(epic_plan** out, int grid_n, int pad, int n_ant, const floa
   }
   if (st == EPIC_OK) st = fused_plan_init(p);
   if (st == EPIC_OK) st = tiled_plan_init(p);
+  if (st == EPIC_OK) st = autocorr_plan_init(p, kernel_taps);
   if (st != EPIC_OK) {
     epic_plan_destroy(p);
     return st;
@@ -288,6 +290,7 @@ int epic_plan_destroy(epic_plan* plan) {
   cudaError_t ce = cudaDeviceSynchronize();
   fused_plan_free(plan);
   tiled_plan_free(plan);
+  autocorr_plan_free(plan);
   if (plan->d_scratch) cudaFree(plan->d_scratch);
   if (plan->d_blob) cudaFree(plan->d_blob);
   delete plan;
@@ -329,6 +332,30 @@ int epic_image(epic_plan* plan, const void* voltages, int n_t, int n_chan, int n
 int epic_image_cf32(epic_plan* plan, const void* voltages_cf32, int n_t, int n_chan, int n_pol,
                     float* out_accum, epic_stream stream) {
   return image_common(plan, voltages_cf32, 1, n_t, n_chan, n_pol, out_accum, stream);
+}
+
+int epic_autocorr_remove(epic_plan* plan, const void* voltages, int n_t, int n_chan, int n_pol,
+                         float* out_accum, epic_stream stream) {
+  if (!plan) return EPIC_ERR_ARG;
+  if (n_t < 0 || n_chan < 0) return EPIC_ERR_ARG;
+  if (n_pol != 1 && n_pol != 2) return EPIC_ERR_RANGE;
+  const int n_products = resolve_products(plan, n_pol);
+  const int n_planes = planes_for(n_pol, n_products);
+  if (n_planes < 0) return EPIC_ERR_RANGE;
+  plan->last_launches = 0;
+  if (n_t == 0 || n_chan == 0) return EPIC_OK;
+  if (!voltages || !out_accum) return EPIC_ERR_ARG;
+  ImageArgs a;
+  a.volt = voltages;
+  a.is_cf32 = 0;
+  a.n_t = n_t;
+  a.n_chan = n_chan;
+  a.n_pol = n_pol;
+  a.n_products = n_products;
+  a.n_planes = n_planes;
+  a.out = out_accum;
+  a.stream = (cudaStream_t)stream;
+  return autocorr_remove(plan, a);
 }
 
 int epic_plan_get_n(const epic_plan* plan) { return plan ? plan->N : (int)EPIC_ERR_ARG; }

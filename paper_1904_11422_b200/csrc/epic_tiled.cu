@@ -23,8 +23,6 @@
 // twiddles (epic_packed.cuh), which come from plan tables computed in double.
 #include <algorithm>
 #include <cmath>
-#include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -394,7 +392,6 @@ int tiled_image_j(epic_plan* p, const ImageArgs& a, TiledParams& P) {
   else st = cols_occupancy<J, 4>(&occ_b, smem_b);
   if (st != EPIC_OK) return st;
   if (occ_a < 1 || occ_b < 1) return EPIC_ERR_RANGE;
-  if (getenv("EPIC_DEBUG")) fprintf(stderr, "tiled: occ_a %d occ_b %d smem_a %zu smem_b %zu max_frames %lld\n", occ_a, occ_b, smem_a, smem_b, max_frames);
   long long Cb = std::min<long long>(a.n_chan, ((long long)occ_b * p->n_sm) / strips);
   Cb = std::max<long long>(1, std::min(Cb, max_frames));
   const long long Tb = std::max<long long>(1, std::min<long long>(n_pairs, max_frames / Cb));

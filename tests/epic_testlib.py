@@ -9,7 +9,8 @@ from oracle import epic_oracle as orc
 TOL = 1e-4  # BASELINE.json north_star: max |gpu - oracle| / image peak, fp32 path
 
 
-def run_gpu(wl, volt=None, path=None, calls=1, n_products=None, return_plan_info=False, scratch_limit=None):
+def run_gpu(wl, volt=None, path=None, calls=1, n_products=None, return_plan_info=False, scratch_limit=None,
+            autocorr=False):
     import torch
     import paper_1904_11422_b200 as epic
 
@@ -34,6 +35,8 @@ def run_gpu(wl, volt=None, path=None, calls=1, n_products=None, return_plan_info
                 plan.image_cf32(part, b - a, wl.n_chan, wl.n_pol, out)
             else:
                 plan.image(part, b - a, wl.n_chan, wl.n_pol, out)
+                if autocorr:  # linear in the gulp: removed per call
+                    plan.autocorr_remove(part, b - a, wl.n_chan, wl.n_pol, out)
         torch.cuda.synchronize()
         info = {"path": plan.path(wl.n_pol), "support": plan.support(), "launches": plan.last_launches()}
         res = out.cpu().numpy()

@@ -235,6 +235,24 @@ def test_results_are_bit_reproducible(wl):
     assert np.array_equal(a, b)
 
 
+# ------------------------------------------------------------------ optional autocorrelation removal
+@pytest.mark.parametrize("wl,calls", [
+    (make_config(2, n_chan=3, n_t=37), 1),                  # fused, delta: flat zero-spacing term
+    (make_config(3, n_chan=2, n_t=29), 2),                  # fused, 3x3 taps, four products, two gulps
+    (make_config(4, n_chan=2, n_t=5), 1),                   # tiled, 256^2
+    (make_custom(grid_n=32, pad=2, n_ant=40, n_pol=1, kernel_k=5, n_chan=2, n_t=11, layout="disc"), 1),
+    (make_custom(grid_n=8, pad=2, n_ant=24, n_pol=2, kernel_k=3, n_chan=1, n_t=6, layout="wrap"), 1),  # two-pass
+], ids=lambda v: v.name if hasattr(v, "name") else str(v))
+def test_autocorr_removal_matches_oracle(wl, calls):
+    """epic_image followed by epic_autocorr_remove equals the oracle's image minus its a = b part
+    (PAPER.md:130), within the image tolerance normalised by the peak of what is LEFT."""
+    v = wl.voltages()
+    gpu = run_gpu(wl, volt=v, calls=calls, autocorr=True)
+    ref = run_oracle(wl, volt=v) - orc.autocorr_image(v, wl.input_kind, wl.ant_uv, wl.taps, wl.grid_n, wl.pad,
+                                                      wl.n_products, kernel_k=wl.kernel_k)
+    assert_parity(gpu, ref, what=f"{wl.name} autocorr removed")
+
+
 def test_calls_accumulate_into_out_accum():
     wl = make_config(2, n_chan=2, n_t=30)
     one = run_gpu(wl, calls=1)

@@ -335,3 +335,47 @@ def test_channel_subset_matches_full_run():
     sub = orc.epic_image(v, "ci4", wl.ant_uv, None, 64, 2, 2, channels=[2, 0], frames_per_batch=3)
     np.testing.assert_allclose(sub[0], full[2], rtol=1e-13)
     np.testing.assert_allclose(sub[1], full[0], rtol=1e-13)
+
+
+# ------------------------------------------------------------------ optional autocorrelation removal
+def test_autocorr_removal_leaves_only_cross_pairs_brute_force():
+    """PAPER.md:130 + Eq. 1-2: with a delta kernel on integer cells the image minus its a = b part
+    is the direct-Fourier image of the visibilities of the pairs a != b only."""
+    rng = np.random.default_rng(11)
+    n, n_ant, t_n = 8, 5, 3
+    cells = rng.choice(n * n, size=n_ant, replace=False)
+    uv = np.stack([cells % n, cells // n], axis=1).astype(np.float32)
+    v = rng.standard_normal((t_n, 1, 2, n_ant, 2)).astype(np.float32)
+    img = orc.epic_image(v, "cf32", uv, None, n, 1, 4)
+    auto = orc.autocorr_image(v, "cf32", uv, None, n, 1, 4)
+    e = v[..., 0].astype(np.float64) + 1j * v[..., 1]
+    x, y = uv[:, 0].astype(int), uv[:, 1].astype(int)
+    ll, mm = np.meshgrid(np.arange(n), np.arange(n), indexing="xy")
+    xx = np.zeros((n, n)); xy = np.zeros((n, n), dtype=complex)
+    for a in range(n_ant):
+        for b in range(n_ant):
+            if a == b:
+                continue
+            ph = np.exp(2j * np.pi * ((x[a] - x[b]) * ll + (y[a] - y[b]) * mm) / n)
+            xx += ((e[:, 0, 0, a] * np.conj(e[:, 0, 0, b])).sum() * ph).real
+            xy += (e[:, 0, 0, a] * np.conj(e[:, 0, 1, b])).sum() * ph
+    got = img[0] - auto[0]
+    assert np.abs(got[0] - xx).max() <= 1e-10 * np.abs(img[0, 0]).max()
+    assert np.abs(got[2] - xy.real).max() <= 1e-10 * np.abs(img[0, 0]).max()
+    assert np.abs(got[3] - xy.imag).max() <= 1e-10 * np.abs(img[0, 0]).max()
+    assert np.allclose(got[4], got[2]) and np.allclose(got[5], -got[3])
+
+
+def test_autocorr_image_special_cases():
+    """One antenna: the whole image is its autocorrelation.  Delta kernel: the a = b part is flat,
+    sum_a sum_t |E_a|^2, whatever the cells."""
+    wl = make_custom(grid_n=8, pad=2, n_ant=1, n_pol=2, kernel_k=3, n_chan=2, n_t=5, n_products=4)
+    v = wl.voltages()
+    img = orc.epic_image(v, "ci4", wl.ant_uv, wl.taps, 8, 2, 4, kernel_k=3)
+    auto = orc.autocorr_image(v, "ci4", wl.ant_uv, wl.taps, 8, 2, 4, kernel_k=3)
+    assert np.abs(img - auto).max() <= 1e-9 * np.abs(img).max()
+    wl = make_custom(grid_n=8, pad=2, n_ant=7, n_pol=1, kernel_k=1, n_chan=1, n_t=4)
+    v = wl.voltages()
+    auto = orc.autocorr_image(v, "ci4", wl.ant_uv, None, 8, 2, 1)
+    flat = (np.abs(orc.unpack_ci4(v)) ** 2).sum()
+    assert np.allclose(auto, flat)
