@@ -201,20 +201,16 @@ __device__ __forceinline__ void row_task(float4* __restrict__ row, const float4*
 }
 
 // columns + S5 + S6: thread = (l1, rho); outputs m = 2Q k + rho, k = 0..15.
-// acc[k] = (|A_lo|^2, |A_hi|^2) sums; xy[k] = sum of A_lo conj(A_hi) (reading Q11) when NPROD == 4.
-template <int NB, int NPROD>
+// acc[k] = (|A_lo|^2, |A_hi|^2) sums in registers (one or two products).
+template <int NB>
 __device__ __forceinline__ void col_task(const float4* __restrict__ col, const float4* __restrict__ tw,
-                                         float2 (&acc)[16], float2 (&xy)[NPROD == 4 ? 16 : 1]) {
+                                         float2 (&acc)[16]) {
   C2 z[16];
   transform32<NB>(z, col, HS, tw);
 #pragma unroll
   for (int k = 0; k < 16; ++k) {
     acc[k] = __ffma2_rn(z[k].re, z[k].re, acc[k]);
     acc[k] = __ffma2_rn(z[k].im, z[k].im, acc[k]);
-    if constexpr (NPROD == 4) {
-      xy[k].x = fmaf(z[k].re.x, z[k].re.y, xy[k].x); xy[k].x = fmaf(z[k].im.x, z[k].im.y, xy[k].x);
-      xy[k].y = fmaf(z[k].im.x, z[k].re.y, xy[k].y); xy[k].y = fmaf(-z[k].re.x, z[k].im.y, xy[k].y);
-    }
   }
 }
 
@@ -259,8 +255,41 @@ __global__ void __launch_bounds__(64 * Q) epic_fused_fixup(FusedParams P, int ma
   }
 }
 
+// Four-product variant: the 64 accumulators of a thread (16 pixels x {XX, YY, Re XY, Im XY}) do not fit
+// beside the 64 data registers at two CTAs per SM, so they are parked in tensor memory (TMEM) and
+// updated 4 pixels at a time: load 16 words, 16 FMAs, store 16 words.  Layout: column 4 k + {0,1,2,3};
+// XY = A_lo conj(A_hi) (reading Q11).
+template <int NB>
+__device__ __forceinline__ void col_task_tmem(const float4* __restrict__ col, const float4* __restrict__ tw,
+                                              uint32_t taddr) {
+  C2 z[16];
+  uint32_t r[2][16];
+  tmem_ld16_issue(taddr, r[0]);  // the first 4 pixels' accumulators travel during the transform
+  transform32<NB>(z, col, HS, tw);
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    tmem_wait_ld();
+    if (c < 3) tmem_ld16_issue(taddr + 16 * (c + 1), r[(c + 1) & 1]);  // next 4 pixels, during this update
+    float a[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) a[i] = __uint_as_float(r[c & 1][i]);
+#pragma unroll
+    for (int kk = 0; kk < 4; ++kk) {
+      const C2& v = z[4 * c + kk];
+      float2 p = make_float2(a[4 * kk], a[4 * kk + 1]);
+      p = __ffma2_rn(v.re, v.re, p);
+      p = __ffma2_rn(v.im, v.im, p);
+      a[4 * kk] = p.x; a[4 * kk + 1] = p.y;
+      a[4 * kk + 2] = fmaf(v.re.x, v.re.y, a[4 * kk + 2]); a[4 * kk + 2] = fmaf(v.im.x, v.im.y, a[4 * kk + 2]);
+      a[4 * kk + 3] = fmaf(v.im.x, v.re.y, a[4 * kk + 3]); a[4 * kk + 3] = fmaf(-v.re.x, v.im.y, a[4 * kk + 3]);
+    }
+    tmem_st16(taddr + 16 * c, a);
+  }
+  tmem_wait_st();
+}
+
 template <int Q, int NPROD, bool DELTA, int NB>
-__global__ void __launch_bounds__(64 * Q, NPROD == 4 ? 1 : 2)
+__global__ void __launch_bounds__(64 * Q, 2)
 epic_fused_kernel(FusedParams P) {
   constexpr int NT = 64 * Q, N = 32 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -273,6 +302,8 @@ epic_fused_kernel(FusedParams P) {
   const long long g0 = P.total * (long long)blockIdx.x / gridDim.x;
   const long long g1 = P.total * (long long)(blockIdx.x + 1) / gridDim.x;
   if (g0 >= g1) return;
+  constexpr bool TMEM = NPROD == 4;        // accumulators in tensor memory
+  constexpr int TCOLS = Q == 4 ? 128 : 64;  // 64 columns per warp; warps w and w + 4 share a lane quadrant
 
   uint2 info[S * S / NT];
 #pragma unroll
@@ -287,12 +318,21 @@ epic_fused_kernel(FusedParams P) {
   const int l1 = (warp & 1) * 16 + (lane >> 1);
   const int rho = (warp >> 1) * 2 + (lane & 1);
 
-  float2 acc[16];
-  float2 xy[NPROD == 4 ? 16 : 1];
+  float2 acc[TMEM ? 1 : 16];
 #pragma unroll
-  for (int k = 0; k < 16; ++k) acc[k] = make_float2(0.0f, 0.0f);
+  for (int k = 0; k < (TMEM ? 1 : 16); ++k) acc[k] = make_float2(0.0f, 0.0f);
+  __shared__ uint32_t tmem_slot;
+  uint32_t tbase = 0u, taddr = 0u;
+  if constexpr (TMEM) {
+    tbase = tmem_alloc_cta<TCOLS>(&tmem_slot, warp);
+    taddr = tbase + (((uint32_t)(warp & 3) * 32u) << 16) + (uint32_t)(warp >> 2) * 64u;
+    float zero[16];
 #pragma unroll
-  for (int k = 0; k < (NPROD == 4 ? 16 : 1); ++k) xy[k] = make_float2(0.0f, 0.0f);
+    for (int i = 0; i < 16; ++i) zero[i] = 0.0f;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) tmem_st16(taddr + 16 * c, zero);
+    tmem_wait_st();
+  }
 
   // S6.  A unit whose whole time range ran in this CTA is added to out_accum directly (this CTA
   // is the only writer of those pixels).  When the equal split of the work list cut a unit's time
@@ -304,15 +344,37 @@ epic_fused_kernel(FusedParams P) {
     const size_t plane = (size_t)N * N;
     float* o = P.out + (size_t)c * P.n_planes * plane + (Q * l1 + l2);
     float* part = P.partial + ((size_t)(blockIdx.x * 2 + slot) * NACC * 16) * NT + tid;
+    if constexpr (TMEM) {
 #pragma unroll
-    for (int k = 0; k < 16; ++k) {
+      for (int c = 0; c < 4; ++c) {
+        float a[16], zero[16];
+        tmem_ld16(taddr + 16 * c, a);
+#pragma unroll
+        for (int i = 0; i < 16; ++i) zero[i] = 0.0f;
+        tmem_st16(taddr + 16 * c, zero);
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk) {
+          const int k = 4 * c + kk;
+          const float v[4] = {a[4 * kk], a[4 * kk + 1], a[4 * kk + 2], a[4 * kk + 3]};
+          if (complete) {
+            add_pixel<4>(o + (size_t)(2 * Q * k + rho) * N, plane, v);
+          } else {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) part[(size_t)(q * 16 + k) * NT] = v[q];
+          }
+        }
+      }
+      tmem_wait_st();
+      return;
+    }
+#pragma unroll
+    for (int k = 0; k < (TMEM ? 1 : 16); ++k) {
       float v[NACC];
       if constexpr (NPROD == 1) {
         v[0] = acc[k].x + acc[k].y;
       } else {
         v[0] = acc[k].x; v[1] = acc[k].y;
       }
-      if constexpr (NPROD == 4) { v[2] = xy[k].x; v[3] = xy[k].y; xy[k] = make_float2(0.0f, 0.0f); }
       acc[k] = make_float2(0.0f, 0.0f);
       if (complete) {
         add_pixel<NPROD>(o + (size_t)(2 * Q * k + rho) * N, plane, v);
@@ -361,7 +423,8 @@ epic_fused_kernel(FusedParams P) {
       // launder the table offset: the twiddles are re-read per task, not held in 18 registers
       int tw_off = rho * TWV;
       asm volatile("" : "+r"(tw_off));
-      col_task<NB, NPROD>(gh + f * PLANE + l1, tws + tw_off, acc, xy);
+      if constexpr (TMEM) col_task_tmem<NB>(gh + f * PLANE + l1, tws + tw_off, taddr);
+      else col_task<NB>(gh + f * PLANE + l1, tws + tw_off, acc);
     }
 
     if (unit_n != unit || !more) {
@@ -371,6 +434,7 @@ epic_fused_kernel(FusedParams P) {
     unit = unit_n; b = b_n;
     __syncthreads();  // next batch's E is complete; gh is free
   }
+  if constexpr (TMEM) tmem_free_cta<TCOLS>(tbase, warp);
 }
 
 struct FusedTables {
@@ -393,6 +457,11 @@ int launch_fused(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
   int per_sm = 0;
   EPIC_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NT, smem));
   if (per_sm < 1) return EPIC_ERR_RANGE;
+  // The occupancy query answers 1 for the kernels that allocate tensor memory, although two CTAs
+  // (128 of the 512 columns each, 128 registers, 2 x 88 KB) do share an SM: measured 22.1 M frames/s
+  // on C3 with 296 CTAs against 18.6 M with 148.  CTAs never wait on one another, so a grid larger
+  // than what is resident would only run as two waves.
+  if (NPROD == 4 && 2 * (smem + 1024) <= (size_t)227 * 1024) per_sm = std::max(per_sm, 2);
   const long long slots = (long long)per_sm * p->n_sm;
   const int grid = (int)std::min<long long>(P.total, slots);
   constexpr int NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
