@@ -32,7 +32,7 @@ UNIT = "frames/s"
 FP32_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # SMs x lanes x FMA x max clock
 L2_FLUSH_BYTES = 256 << 20
 PATH_NAMES = {1: "twopass", 2: "fused", 3: "tiled"}
-PATH_KERNELS = {1: "grid_rowfft+colfft_accum", 2: "epic_fused_kernel", 3: "tiled_rows+tiled_cols"}
+PATH_KERNELS = {1: "grid_rowfft+colfft_accum", 2: "epic_fused_kernel (+ epic_fused_fixup, <1 % of the step)", 3: "tiled_rows+tiled_cols"}
 
 
 def algorithmic_flops_per_frame(wl) -> float:
