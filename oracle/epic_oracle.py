@@ -252,3 +252,39 @@ def autocorr_image(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Op
                 out[ci, 2], out[ci, 3] = xy.real, xy.imag
                 out[ci, 4], out[ci, 5] = xy.real, -xy.imag
     return out
+
+
+# ------------------------------------------------------------------ sampled outputs at any size
+def pixel_values(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Optional[np.ndarray],
+                 grid_n: int, pad: int, n_products: int, pixels, kernel_k: int = 1,
+                 channels: Optional[list] = None) -> np.ndarray:
+    """Accumulated image values at a few pixels, float64 [C'][planes][len(pixels)], straight from
+    the discretised Eq. 5 one pixel at a time, with no grid and no FFT:
+
+        A_p(t)[m][l] = sum_a E_ap(t) * sum_d W_a[d] exp(+2 pi i ((cx_a+dx) l + (cy_a+dy) m) / N)
+
+    (cells modulo N, reading Q6), then the products summed over t.  Cost O(T * A) per pixel, so it
+    checks sampled outputs of full-size configurations that epic_image() cannot finish in
+    reasonable time.  ``pixels`` is a list of (m, l)."""
+    n = grid_n * pad
+    t_n, c_n, n_pol, n_ant = voltages.shape[:4]
+    ch = list(range(c_n)) if channels is None else list(channels)
+    cells = tap_cells(ant_uv, kernel_k, n)          # [A][K][K] flat y*N + x
+    w = taps_to_complex(taps, n_ant, kernel_k)      # [A][K][K]
+    cy, cx = cells // n, cells % n
+    pl = n_planes(n_pol, n_products)
+    out = np.zeros((len(ch), pl, len(pixels)), dtype=np.float64)
+    for pi, (m, l) in enumerate(pixels):
+        phase = np.exp(1j * TWO_PI * ((cx * l + cy * m) % n) / n)
+        u = (w * phase).sum(axis=(1, 2))            # [A]: response of antenna a at this pixel
+        for ci, c in enumerate(ch):
+            e = voltages_to_complex(voltages[:, c], kind)   # [T][Np][A]
+            a = e @ u                                        # [T][Np]
+            out[ci, 0, pi] = (np.abs(a[:, 0]) ** 2).sum()
+            if n_pol == 2:
+                out[ci, 1, pi] = (np.abs(a[:, 1]) ** 2).sum()
+                if n_products == 4:
+                    xy = (a[:, 0] * np.conj(a[:, 1])).sum()
+                    out[ci, 2, pi], out[ci, 3, pi] = xy.real, xy.imag
+                    out[ci, 4, pi], out[ci, 5, pi] = xy.real, -xy.imag
+    return out

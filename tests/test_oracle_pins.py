@@ -379,3 +379,23 @@ def test_autocorr_image_special_cases():
     auto = orc.autocorr_image(v, "ci4", wl.ant_uv, None, 8, 2, 1)
     flat = (np.abs(orc.unpack_ci4(v)) ** 2).sum()
     assert np.allclose(auto, flat)
+
+
+# ------------------------------------------------------------------ sampled outputs
+@pytest.mark.parametrize("wl", [
+    make_config(1),
+    make_custom(grid_n=8, pad=2, n_ant=24, n_pol=2, kernel_k=3, n_chan=2, n_t=5, layout="wrap"),
+    make_custom(grid_n=16, pad=2, n_ant=9, n_pol=1, kernel_k=5, n_chan=1, n_t=4, input_kind="cf32"),
+], ids=lambda w: w.name)
+def test_pixel_values_equal_the_imaged_pixels(wl):
+    """pixel_values (Eq. 5 written out for one pixel: no grid, no FFT) against epic_image in
+    definition mode (the literal double sum over the gridded plane) on every plane."""
+    v = wl.voltages()
+    img = orc.epic_image(v, wl.input_kind, wl.ant_uv, wl.taps, wl.grid_n, wl.pad, wl.n_products,
+                         kernel_k=wl.kernel_k, mode="definition" if wl.N <= 16 else "fast")
+    rng = np.random.default_rng(3)
+    pix = [(0, 0), (wl.N - 1, 1)] + [tuple(int(x) for x in rng.integers(0, wl.N, 2)) for _ in range(6)]
+    got = orc.pixel_values(v, wl.input_kind, wl.ant_uv, wl.taps, wl.grid_n, wl.pad, wl.n_products, pix,
+                           kernel_k=wl.kernel_k)
+    for i, (m, l) in enumerate(pix):
+        assert np.abs(got[:, :, i] - img[:, :, m, l]).max() <= 1e-10 * np.abs(img).max()
