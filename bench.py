@@ -117,13 +117,13 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def cpu_baseline(wl, volt, n_chan_sample: int) -> dict:
+def cpu_baseline(wl, volt, n_chan_sample: int, order: str = "TCPA") -> dict:
     """The float64 oracle, as it stands, on a bounded sample of the same workload."""
     from oracle import epic_oracle as orc
     ch = list(range(min(n_chan_sample, wl.n_chan)))
     t0 = time.perf_counter()
     orc.epic_image(volt, wl.input_kind, wl.ant_uv, wl.taps, wl.grid_n, wl.pad, wl.n_products,
-                   kernel_k=wl.kernel_k, mode="fast", channels=ch)
+                   kernel_k=wl.kernel_k, mode="fast", channels=ch, order=order)
     dt = time.perf_counter() - t0
     frames = len(ch) * volt.shape[0]
     return {"value": frames / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
@@ -176,6 +176,8 @@ def run_epic(args, wl):
     dev = torch.device("cuda", local)
 
     volt = wl.voltages()                       # host, seeded synthetic (DESIGN.md input recipe)
+    if args.input_order == "tcap":             # the untransposed F-engine order
+        volt = np.ascontiguousarray(np.swapaxes(volt, 2, 3))
     h_volt = torch.from_numpy(volt).pin_memory()
     d_volt = h_volt.to(dev, non_blocking=True)
     plan = epic.Plan(wl.grid_n, wl.pad, wl.ant_uv, wl.taps, wl.kernel_k)
@@ -184,6 +186,11 @@ def run_epic(args, wl):
         plan.set_path({"auto": 0, "twopass": 1, "fused": 2, "tiled": 3}[args.path])
     if args.scratch_mib:
         plan.set_scratch_limit(args.scratch_mib << 20)
+    if args.input_order == "tcap":
+        plan.set_input_order(epic.EPIC_ORDER_TCAP)
+    if args.delay_phasors:                     # unit-modulus synthetic cable phases
+        ph_rng = np.random.default_rng(wl.seed + 77)
+        plan.set_delay_phasors(np.exp(2j * np.pi * ph_rng.random((wl.n_chan, wl.n_pol, wl.n_ant))).astype(np.complex64))
     planes = plan.n_planes(wl.n_pol)
     out = torch.zeros((wl.n_chan, planes, wl.N, wl.N), dtype=torch.float32, device=dev)
     h_out = torch.empty(out.shape, dtype=torch.float32).pin_memory()
@@ -289,6 +296,7 @@ def run_epic(args, wl):
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": wl.name, **{k: v for k, v in wl.describe().items() if k != "workload"},
                    "kernel_path": PATH_NAMES.get(path, str(path)),
+                   "input_order": args.input_order, "delay_phasors": bool(args.delay_phasors),
                    "support_box": list(support), "l2": f"flushed between iterations ({L2_FLUSH_BYTES >> 20} MiB write)",
                    "sharding": "independent replicas of the workload per GPU (channels are independent), no collective"},
         "roofline": {
@@ -307,7 +315,7 @@ def run_epic(args, wl):
         "clocks": clocks,
     }
     if world == 1 and not args.no_cpu_baseline:
-        line["cpu_baseline"] = cpu_baseline(wl, volt, args.cpu_channels)
+        line["cpu_baseline"] = cpu_baseline(wl, volt, args.cpu_channels, args.input_order.upper())
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -326,6 +334,8 @@ def main():
     ap.add_argument("--n-ant", type=int, default=None)
     ap.add_argument("--cpu-channels", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--input-order", default="tcpa", choices=["tcpa", "tcap"], help="tcap = [T][C][A][Np], transposed in the load")
+    ap.add_argument("--delay-phasors", action="store_true", help="apply per-(channel, pol, antenna) delay phasors")
     ap.add_argument("--e2e-chunks", type=int, default=4, help="time chunks of the end-to-end leg (H2D overlapped)")
     ap.add_argument("--scratch-mib", type=int, default=0, help="cap the per-batch scratch (tiled / two-pass paths)")
     args = ap.parse_args()

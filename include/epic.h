@@ -104,6 +104,22 @@ EPIC_API int epic_image(epic_plan* plan, const void* voltages, int n_t, int n_ch
 EPIC_API int epic_image_cf32(epic_plan* plan, const void* voltages_cf32, int n_t, int n_chan, int n_pol,
                     float* out_accum, epic_stream stream);
 
+/* Upstream steps folded into the load.
+ * Input order: the F-engine packets arrive as [Time, Channel, Antenna, Polarisation]; the paper
+ * transposes them to [Time, Channel, Polarisation, Antenna] before gridding.  With
+ * EPIC_ORDER_TCAP epic_image / epic_image_cf32 / epic_autocorr_remove read the untransposed order
+ * directly (the transposition happens in the kernels' staging loads).  Default EPIC_ORDER_TCPA. */
+typedef enum epic_order { EPIC_ORDER_TCPA = 0, EPIC_ORDER_TCAP = 1 } epic_order;
+EPIC_API int epic_plan_set_input_order(epic_plan* plan, int order);
+
+/* Delay compensation ("compensation for the signal path delays are applied"): every
+ * unpacked voltage of (channel c, polarisation p, antenna a) is multiplied by the complex number
+ * phasors[c][p][a] before gridding (typically exp(-2 pi i nu_c tau_a); computing it is the caller's
+ * business, as it was the LWA library's in the paper).
+ *   phasors  HOST float[n_chan][n_pol][n_ant][2] (re, im), copied; NULL removes the table.
+ * While a table is set, image calls must use the same n_chan and n_pol (else EPIC_ERR_ARG). */
+EPIC_API int epic_plan_set_delay_phasors(epic_plan* plan, int n_chan, int n_pol, const float* phasors);
+
 /* Optional autocorrelation removal ("to remove the zero-spacing power inherent in EPIC";
  * SURVEY.md 8(f) NEXT-2).  The EPIC image of a gulp is the direct-Fourier image of ALL antenna pairs,
  * a = b included; this call SUBTRACTS from out_accum the a = b part of the same gulp,

@@ -25,7 +25,8 @@ Readings of the paper where it is silent (SURVEY.md §8(c)
 Q1 high nibble real / low nibble imaginary, two's complement; Q4 nearest cell = floor(x+0.5);
 Q6 cells wrap modulo N; Q8 +2 pi i (inverse transform); Q9 unnormalised; Q10 natural order,
 zenith at [0][0]; Q11 XY = A_X conj(A_Y); Q12 plain sum over time; Q14 plane order
-{XX} | {XX,YY} | {XX,YY,ReXY,ImXY,ReYX,ImYX}.
+{XX} | {XX,YY} | {XX,YY,ReXY,ImXY,ReYX,ImYX}; Q19 delay compensation = one complex multiplier per
+(channel, pol, antenna) applied after unpack.
 
 Pins (tests/test_oracle_*.py, all ``-m "not gpu"``): S1 exhaustive nibble table typed out in the
 test; S2 hand-worked cells incl. half-cells and wrap; S3 closed-form sums, collisions add,
@@ -70,6 +71,24 @@ def voltages_to_complex(v: np.ndarray, kind: str) -> np.ndarray:
         v = np.asarray(v, dtype=np.float32).astype(np.float64)
         return v[..., 0] + 1j * v[..., 1]
     raise ValueError(kind)
+
+
+def channel_voltages(voltages: np.ndarray, kind: str, c: int, t0: int = 0, t1: Optional[int] = None,
+                     order: str = "TCPA", delay_phasors: Optional[np.ndarray] = None) -> np.ndarray:
+    """complex128 [t1-t0][Np][A] of channel c, ready for gridding: the steps upstream of it in the
+    paper's pipeline.  ``order`` "TCAP" = the F-engine order [Time, Channel, Antenna, Polarisation]
+    that the paper's transposition block turns into [Time, Channel, Polarisation, Antenna]
+    (PAPER.md:120); ``delay_phasors`` complex [C][Np][A] = the "compensation for the signal path
+    delays" (PAPER.md:122), read as one complex multiplier per (channel, pol, antenna) (Q19)."""
+    v = voltages[t0:t1, c]
+    if order == "TCAP":
+        v = np.swapaxes(v, 1, 2)        # [t][A][Np] -> [t][Np][A]
+    elif order != "TCPA":
+        raise ValueError(order)
+    e = voltages_to_complex(v, kind)
+    if delay_phasors is not None:
+        e = e * np.asarray(delay_phasors, dtype=np.complex128)[c][None, :, :]
+    return e
 
 
 # ------------------------------------------------------------------ S2: cells
@@ -187,7 +206,8 @@ def products(a: np.ndarray, n_products: int) -> np.ndarray:
 def epic_image(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Optional[np.ndarray],
                grid_n: int, pad: int, n_products: int, kernel_k: int = 1,
                mode: str = "fast", channels: Optional[list] = None,
-               frames_per_batch: Optional[int] = None) -> np.ndarray:
+               frames_per_batch: Optional[int] = None, order: str = "TCPA",
+               delay_phasors: Optional[np.ndarray] = None) -> np.ndarray:
     """Accumulated polarised images, float64 [C'][planes][N][N] (C' = len(channels) or C).
 
     voltages: ci4 uint8 [T][C][Np][A] or cf32 float32 [T][C][Np][A][2] (PAPER.md:120 order
@@ -196,7 +216,8 @@ def epic_image(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Option
     (used for sampled parity at full size; channels are independent).
     """
     n = grid_n * pad
-    t_n, c_n, n_pol, n_ant = voltages.shape[:4]
+    t_n, c_n = voltages.shape[:2]
+    n_pol, n_ant = (voltages.shape[3], voltages.shape[2]) if order == "TCAP" else voltages.shape[2:4]
     ch = list(range(c_n)) if channels is None else list(channels)
     cells = tap_cells(ant_uv, kernel_k, n)
     w = taps_to_complex(taps, n_ant, kernel_k)
@@ -207,7 +228,7 @@ def epic_image(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Option
         frames_per_batch = max(1, min(t_n, (1 << 21) // (n * n * n_pol)))
     for ci, c in enumerate(ch):
         for t0 in range(0, t_n, frames_per_batch):
-            e = voltages_to_complex(voltages[t0:t0 + frames_per_batch, c], kind)  # [F][Np][A]
+            e = channel_voltages(voltages, kind, c, t0, t0 + frames_per_batch, order, delay_phasors)  # [F][Np][A]
             f = e.shape[0]
             img = np.empty((f, n_pol, n, n), dtype=np.complex128)
             for p in range(n_pol):
@@ -220,7 +241,8 @@ def epic_image(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Option
 # ------------------------------------------------------------------ optional: autocorrelation removal
 def autocorr_image(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Optional[np.ndarray],
                    grid_n: int, pad: int, n_products: int, kernel_k: int = 1,
-                   channels: Optional[list] = None) -> np.ndarray:
+                   channels: Optional[list] = None, order: str = "TCPA",
+                   delay_phasors: Optional[np.ndarray] = None) -> np.ndarray:
     """The a = b part of the accumulated EPIC image ("the zero-spacing power inherent in
     EPIC"), float64 [C'][planes][N][N], from the definition: the image is
     sum_t A_p conj(A_q) with A_p = sum_a E_ap What_a, What_a = transform of antenna a gridded alone
@@ -228,7 +250,8 @@ def autocorr_image(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Op
     Subtracting it from epic_image leaves the direct-Fourier image of the pairs a != b only
     (pinned in tests/test_oracle_pins.py by brute force)."""
     n = grid_n * pad
-    t_n, c_n, n_pol, n_ant = voltages.shape[:4]
+    t_n, c_n = voltages.shape[:2]
+    n_pol, n_ant = (voltages.shape[3], voltages.shape[2]) if order == "TCAP" else voltages.shape[2:4]
     ch = list(range(c_n)) if channels is None else list(channels)
     cells = tap_cells(ant_uv, kernel_k, n)
     w = taps_to_complex(taps, n_ant, kernel_k)
@@ -240,7 +263,7 @@ def autocorr_image(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Op
     pl = n_planes(n_pol, n_products)
     out = np.zeros((len(ch), pl, n, n), dtype=np.float64)
     for ci, c in enumerate(ch):
-        e = voltages_to_complex(voltages[:, c], kind)  # [T][Np][A]
+        e = channel_voltages(voltages, kind, c, 0, None, order, delay_phasors)  # [T][Np][A]
         vxx = (np.abs(e[:, 0]) ** 2).sum(axis=0)       # [A]
         out[ci, 0] = np.tensordot(vxx, beam, axes=1)
         if n_pol == 2:
@@ -257,7 +280,8 @@ def autocorr_image(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Op
 # ------------------------------------------------------------------ sampled outputs at any size
 def pixel_values(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Optional[np.ndarray],
                  grid_n: int, pad: int, n_products: int, pixels, kernel_k: int = 1,
-                 channels: Optional[list] = None) -> np.ndarray:
+                 channels: Optional[list] = None, order: str = "TCPA",
+                 delay_phasors: Optional[np.ndarray] = None) -> np.ndarray:
     """Accumulated image values at a few pixels, float64 [C'][planes][len(pixels)], straight from
     the discretised Eq. 5 one pixel at a time, with no grid and no FFT:
 
@@ -267,7 +291,8 @@ def pixel_values(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Opti
     checks sampled outputs of full-size configurations that epic_image() cannot finish in
     reasonable time.  ``pixels`` is a list of (m, l)."""
     n = grid_n * pad
-    t_n, c_n, n_pol, n_ant = voltages.shape[:4]
+    t_n, c_n = voltages.shape[:2]
+    n_pol, n_ant = (voltages.shape[3], voltages.shape[2]) if order == "TCAP" else voltages.shape[2:4]
     ch = list(range(c_n)) if channels is None else list(channels)
     cells = tap_cells(ant_uv, kernel_k, n)          # [A][K][K] flat y*N + x
     w = taps_to_complex(taps, n_ant, kernel_k)      # [A][K][K]
@@ -278,7 +303,7 @@ def pixel_values(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Opti
         phase = np.exp(1j * TWO_PI * ((cx * l + cy * m) % n) / n)
         u = (w * phase).sum(axis=(1, 2))            # [A]: response of antenna a at this pixel
         for ci, c in enumerate(ch):
-            e = voltages_to_complex(voltages[:, c], kind)   # [T][Np][A]
+            e = channel_voltages(voltages, kind, c, 0, None, order, delay_phasors)   # [T][Np][A]
             a = e @ u                                        # [T][Np]
             out[ci, 0, pi] = (np.abs(a[:, 0]) ** 2).sum()
             if n_pol == 2:

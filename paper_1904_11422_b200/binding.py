@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(_PKG, "libepic.so")
 EPIC_OK = 0
 EPIC_ERR_ARG, EPIC_ERR_RANGE, EPIC_ERR_CUDA, EPIC_ERR_NOMEM = -1, -2, -3, -4
 EPIC_PATH_AUTO, EPIC_PATH_TWOPASS, EPIC_PATH_FUSED, EPIC_PATH_TILED = 0, 1, 2, 3
+EPIC_ORDER_TCPA, EPIC_ORDER_TCAP = 0, 1
 
 # every symbol include/epic.h declares: name -> (restype, argtypes)
 _vp, _i, _l = ctypes.c_void_p, ctypes.c_int, ctypes.c_long
@@ -25,6 +26,8 @@ SYMBOLS = {
     "epic_plan_set_products": (_i, [_vp, _i]),
     "epic_plan_set_path": (_i, [_vp, _i]),
     "epic_plan_set_scratch_limit": (_i, [_vp, ctypes.c_longlong]),
+    "epic_plan_set_input_order": (_i, [_vp, _i]),
+    "epic_plan_set_delay_phasors": (_i, [_vp, _i, _i, _vp]),
     "epic_image": (_i, [_vp, _vp, _i, _i, _i, _vp, _vp]),
     "epic_image_cf32": (_i, [_vp, _vp, _i, _i, _i, _vp, _vp]),
     "epic_autocorr_remove": (_i, [_vp, _vp, _i, _i, _i, _vp, _vp]),
@@ -140,6 +143,24 @@ class Plan:
     # -- configuration / queries
     def set_products(self, n_products: int) -> None:
         _check(lib().epic_plan_set_products(self._h, n_products), "epic_plan_set_products")
+
+    def set_input_order(self, order: int) -> None:
+        """EPIC_ORDER_TCPA (default) or EPIC_ORDER_TCAP: voltages in [T][C][A][Np] order (PAPER.md:120)."""
+        _check(lib().epic_plan_set_input_order(self._h, int(order)), "epic_plan_set_input_order")
+
+    def set_delay_phasors(self, phasors: Optional[np.ndarray]) -> None:
+        """HOST complex multipliers [n_chan][n_pol][n_ant] (complex64, or float32 [...][2]); None clears."""
+        if phasors is None:
+            _check(lib().epic_plan_set_delay_phasors(self._h, 0, 0, 0), "epic_plan_set_delay_phasors")
+            return
+        ph = np.asarray(phasors)
+        if np.iscomplexobj(ph):
+            ph = np.stack([ph.real, ph.imag], axis=-1)
+        ph = np.ascontiguousarray(ph, dtype=np.float32)
+        if ph.ndim != 4 or ph.shape[2] != self.n_ant or ph.shape[3] != 2:
+            raise ValueError(f"phasors shape {ph.shape}")
+        _check(lib().epic_plan_set_delay_phasors(self._h, ph.shape[0], ph.shape[1], _ptr(ph)),
+               "epic_plan_set_delay_phasors")
 
     def set_scratch_limit(self, n_bytes: int):
         _check(lib().epic_plan_set_scratch_limit(self._h, int(n_bytes)), "epic_plan_set_scratch_limit")

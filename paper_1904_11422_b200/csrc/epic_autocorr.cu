@@ -35,7 +35,7 @@ __device__ __forceinline__ int sext4_lo(uint32_t b) { return ((int)(int8_t)((b <
 // One thread follows VEC consecutive antennas (VEC = 4: aligned 32-bit loads) through the chunk's samples.
 template <int VEC>
 __global__ void __launch_bounds__(128) autocorr_power(const uint8_t* __restrict__ volt, int n_t, int n_chan,
-                                                      int n_pol, int n_ant, int4* __restrict__ power) {
+                                                      int n_pol, int n_ant, int native, int4* __restrict__ power) {
   const int chunk = blockIdx.x, c = blockIdx.y;
   const int t0 = (int)((long long)n_t * chunk / CHUNKS), t1 = (int)((long long)n_t * (chunk + 1) / CHUNKS);
   const size_t row = (size_t)n_pol * n_ant, step = (size_t)n_chan * row;
@@ -43,10 +43,20 @@ __global__ void __launch_bounds__(128) autocorr_power(const uint8_t* __restrict_
     int xx[VEC], yy[VEC], xyr[VEC], xyi[VEC];
 #pragma unroll
     for (int i = 0; i < VEC; ++i) xx[i] = yy[i] = xyr[i] = xyi[i] = 0;
-    const uint8_t* p = volt + ((size_t)t0 * n_chan + c) * row + a;
+    const bool tcap = native && n_pol == 2;  // untransposed order: (a X, a Y) byte pairs
+    const uint8_t* p = volt + ((size_t)t0 * n_chan + c) * row + (tcap ? 2 * a : a);
     for (int t = t0; t < t1; ++t, p += step) {
       uint32_t wx, wy = 0u;
-      if (VEC == 4) {
+      if (tcap) {
+        if (VEC == 4) {
+          const uint32_t w0 = __ldg(reinterpret_cast<const uint32_t*>(p)), w1 = __ldg(reinterpret_cast<const uint32_t*>(p) + 1);
+          wx = __byte_perm(w0, w1, 0x6420u);
+          wy = __byte_perm(w0, w1, 0x7531u);
+        } else {
+          wx = __ldg(p);
+          wy = __ldg(p + 1);
+        }
+      } else if (VEC == 4) {
         wx = __ldg(reinterpret_cast<const uint32_t*>(p));
         if (n_pol == 2) wy = __ldg(reinterpret_cast<const uint32_t*>(p + n_ant));
       } else {
@@ -70,8 +80,9 @@ __global__ void __launch_bounds__(128) autocorr_power(const uint8_t* __restrict_
 }
 
 // psum[c * A + a] = chunk-summed power as floats (the integer sums are exact; the order is fixed)
+// With delay phasors d (reading Q19) the compensated powers are |d_x|^2 xx, |d_y|^2 yy, d_x conj(d_y) xy.
 __global__ void __launch_bounds__(256) autocorr_sum(const int4* __restrict__ power, int n_chan, int n_ant,
-                                                    float4* __restrict__ psum) {
+                                                    const float4* __restrict__ phasor, float4* __restrict__ psum) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n_chan * n_ant) return;
   const int c = i / n_ant, a = i - c * n_ant;
@@ -81,7 +92,13 @@ __global__ void __launch_bounds__(256) autocorr_sum(const int4* __restrict__ pow
     const int4 v = __ldg(power + ((size_t)c * CHUNKS + k) * n_ant + a);
     xx += v.x; yy += v.y; xyr += v.z; xyi += v.w;
   }
-  psum[i] = make_float4((float)xx, (float)yy, (float)xyr, (float)xyi);
+  float4 v = make_float4((float)xx, (float)yy, (float)xyr, (float)xyi);
+  if (phasor) {
+    const float4 d = __ldg(phasor + i);  // (re_x, re_y, im_x, im_y)
+    const float gr = d.x * d.y + d.z * d.w, gi = d.z * d.y - d.x * d.w;  // d_x conj(d_y)
+    v = make_float4(v.x * (d.x * d.x + d.z * d.z), v.y * (d.y * d.y + d.w * d.w), v.z * gr - v.w * gi, v.z * gi + v.w * gr);
+  }
+  psum[i] = v;
 }
 
 // lags[(c * n_lag + q) * 6] = (Lxx.re, Lxx.im, Lyy.re, Lyy.im, Lxy.re, Lxy.im) = sum_a V_aa corr_a[q].
@@ -206,12 +223,12 @@ int autocorr_remove(epic_plan* p, const ImageArgs& a) {
   const uint8_t* volt = static_cast<const uint8_t*>(a.volt);
   if (A % 4 == 0 && (reinterpret_cast<uintptr_t>(volt) & 3u) == 0) {
     const int gz = std::max(1, std::min(8, A / 4 / 128));
-    autocorr_power<4><<<dim3(CHUNKS, a.n_chan, gz), 128, 0, a.stream>>>(volt, a.n_t, a.n_chan, a.n_pol, A, power);
+    autocorr_power<4><<<dim3(CHUNKS, a.n_chan, gz), 128, 0, a.stream>>>(volt, a.n_t, a.n_chan, a.n_pol, A, a.native, power);
   } else {
     const int gz = std::max(1, std::min(8, A / 128));
-    autocorr_power<1><<<dim3(CHUNKS, a.n_chan, gz), 128, 0, a.stream>>>(volt, a.n_t, a.n_chan, a.n_pol, A, power);
+    autocorr_power<1><<<dim3(CHUNKS, a.n_chan, gz), 128, 0, a.stream>>>(volt, a.n_t, a.n_chan, a.n_pol, A, a.native, power);
   }
-  autocorr_sum<<<(a.n_chan * A + 255) / 256, 256, 0, a.stream>>>(power, a.n_chan, A, psum);
+  autocorr_sum<<<(a.n_chan * A + 255) / 256, 256, 0, a.stream>>>(power, a.n_chan, A, a.phasor_pair, psum);
   autocorr_lags<<<dim3(a.n_chan, (n_lag + 3) / 4), 128, 0, a.stream>>>(psum, at->corr, A, n_lag, lags);
   autocorr_subtract<<<dim3((N * N + 255) / 256, a.n_chan), 256, 0, a.stream>>>(lags, p->t.twiddle, N, K, a.n_planes,
                                                                               a.out);

@@ -94,6 +94,8 @@ struct FusedParams {
   const float2* ent_tap;
   const float4* tw;          // [2Q][TWV]: the TwSet of every residue rho
   float* partial;            // scratch [grid][2 slots][NACC][16][NT]: partial sums of split units
+  int native;                // input order [T][C][A][Np] instead of [T][C][Np][A]
+  const float4* phasor;      // delay phasors, pair-packed [C][A], or nullptr
   int n_t, n_chan, n_ant, n_pol, n_planes;
   int R, Cc;                 // occupied rows / columns of the block
   int nb;                    // batches per unit
@@ -129,6 +131,14 @@ __device__ __forceinline__ void prefetch_batch(const FusedParams& P, const Prefe
     wlo[k] = 0u; whi[k] = 0u;
     if (ps.j[k] >= 0) {
       const int t_lo = (b * F + ps.j[k]) * tmul, t_hi = t_lo + thi;
+      if (P.native && P.n_pol == 2) {  // (a X, a Y) byte pairs: two words hold this slot's four antennas
+        if (t_lo < P.n_t) {
+          const uint32_t* src = reinterpret_cast<const uint32_t*>(
+              P.volt + ((size_t)t_lo * P.n_chan + c) * row_bytes + 2 * ps.a[k]);
+          deinterleave_pols(__ldg(src), __ldg(src + 1), wlo[k], whi[k]);
+        }
+        continue;
+      }
       const uint8_t* base = P.volt + (size_t)c * row_bytes + ps.a[k];
       if (t_lo < P.n_t) wlo[k] = __ldg(reinterpret_cast<const uint32_t*>(base + (size_t)t_lo * P.n_chan * row_bytes));
       if (t_hi < P.n_t) whi[k] = __ldg(reinterpret_cast<const uint32_t*>(base + (size_t)t_hi * P.n_chan * row_bytes + hi_off));
@@ -138,10 +148,12 @@ __device__ __forceinline__ void prefetch_batch(const FusedParams& P, const Prefe
 
 // registers -> E[F][A] (float4 per antenna), S1
 __device__ __forceinline__ void unpack_batch(const FusedParams& P, const PrefetchSlots& ps, float4* __restrict__ E,
-                                             const uint32_t (&wlo)[MAXW], const uint32_t (&whi)[MAXW]) {
+                                             const uint32_t (&wlo)[MAXW], const uint32_t (&whi)[MAXW], int c) {
 #pragma unroll
   for (int k = 0; k < MAXW; ++k)
-    if (ps.j[k] >= 0) unpack_words(wlo[k], whi[k], E + ps.j[k] * P.n_ant + ps.a[k], (int)(threadIdx.x >> 1));
+    if (ps.j[k] >= 0)
+      unpack_words(wlo[k], whi[k], E + ps.j[k] * P.n_ant + ps.a[k], (int)(threadIdx.x >> 1),
+                   P.phasor ? P.phasor + (size_t)c * P.n_ant + ps.a[k] : nullptr);
 }
 
 // S3 for the batch: every thread owns the cell slots tid + j*NT of the plan's list and sums their
@@ -393,7 +405,7 @@ epic_fused_kernel(FusedParams P) {
   prefetch_init<NT>(P, tid, ps);
   uint32_t wlo[MAXW], whi[MAXW];
   prefetch_batch<NT>(P, ps, unit / Q, b, wlo, whi);
-  unpack_batch(P, ps, E, wlo, whi);
+  unpack_batch(P, ps, E, wlo, whi, unit / Q);
   __syncthreads();
 
   const int ntask = F * P.R * 2;
@@ -417,7 +429,7 @@ epic_fused_kernel(FusedParams P) {
     }
     __syncthreads();
 
-    if (more) unpack_batch(P, ps, E, wlo, whi);  // E was last read by this batch's gather
+    if (more) unpack_batch(P, ps, E, wlo, whi, unit_n / Q);  // E was last read by this batch's gather
 #pragma unroll 1
     for (int f = 0; f < F; ++f) {
       // launder the table offset: the twiddles are re-read per task, not held in 18 registers
@@ -588,6 +600,8 @@ int fused_image(epic_plan* p, const ImageArgs& a) {
   P.ent_tap = p->t.ent_tap;
   P.tw = ft->tw;
   P.partial = static_cast<float*>(p->d_scratch);
+  P.native = a.native;
+  P.phasor = a.phasor_pair;
   P.n_t = a.n_t;
   P.n_chan = a.n_chan;
   P.n_ant = p->n_ant;

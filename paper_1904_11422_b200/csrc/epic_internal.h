@@ -45,6 +45,10 @@ struct epic_plan {
   int fused_ok;                // support fits the fused kernel
   void* d_tiled;               // tables private to the tiled path
   void* d_auto;                // tap autocorrelation table of epic_autocorr_remove
+  int input_order;             // EPIC_ORDER_TCPA | EPIC_ORDER_TCAP
+  int ph_n_chan, ph_n_pol;     // shape of the delay phasor table (0: none set)
+  float2* d_phasor;            // [ph_n_chan][ph_n_pol][n_ant] complex multipliers (reading Q19)
+  float4* d_phasor_pair;       // [ph_n_chan][n_ant] (re_lo, re_hi, im_lo, im_hi): lo/hi = pol X/Y, or the same pol twice
   int tiled_ok;                // N is 256 or 512
   int n_sm;
   // host copies kept for the fused path's table builder
@@ -58,6 +62,9 @@ namespace epic {
 struct ImageArgs {
   const void* volt;
   int is_cf32;
+  int native;                  // voltages in [T][C][A][Np] order (else [T][C][Np][A])
+  const float2* phasor;        // delay phasors [C][Np][A] or nullptr
+  const float4* phasor_pair;   // the same, pair-packed [C][A], or nullptr
   int n_t, n_chan, n_pol, n_products, n_planes;
   float* out;
   cudaStream_t stream;

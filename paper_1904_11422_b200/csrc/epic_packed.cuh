@@ -93,8 +93,11 @@ __device__ __forceinline__ float biased_byte_to_float_bits(uint32_t w, int i) {
   return __uint_as_float(__byte_perm(w, 0x4B400000u, 0x7650u + (uint32_t)i));
 }
 
-// word pair (lo plane, hi plane) of antennas a0..a0+3 -> E[a0..a0+3] = (re_lo, re_hi, im_lo, im_hi)
-__device__ __forceinline__ void unpack_words(uint32_t wlo, uint32_t whi, float4* __restrict__ e, int rot) {
+// word pair (lo plane, hi plane) of antennas a0..a0+3 -> E[a0..a0+3] = (re_lo, re_hi, im_lo, im_hi).
+// `ph` (or nullptr): the four antennas' delay phasors, pair-packed the same way; each sample is
+// multiplied by its phasor (PAPER.md:122 delay compensation; reading Q19).
+__device__ __forceinline__ void unpack_words(uint32_t wlo, uint32_t whi, float4* __restrict__ e, int rot,
+                                             const float4* __restrict__ ph = nullptr) {
   const uint32_t rl = ((wlo >> 4) & 0x0F0F0F0Fu) ^ 0x08080808u, il = (wlo & 0x0F0F0F0Fu) ^ 0x08080808u;
   const uint32_t rh = ((whi >> 4) & 0x0F0F0F0Fu) ^ 0x08080808u, ih = (whi & 0x0F0F0F0Fu) ^ 0x08080808u;
   const float2 bias = f2(-12582920.0f);
@@ -102,10 +105,24 @@ __device__ __forceinline__ void unpack_words(uint32_t wlo, uint32_t whi, float4*
   for (int k = 0; k < 4; ++k) {
     // lanes store their four cells in rotated order so that a quarter-warp covers all 8 bank groups
     const int i = (k + rot) & 3;
-    const float2 re = __fadd2_rn(make_float2(biased_byte_to_float_bits(rl, i), biased_byte_to_float_bits(rh, i)), bias);
-    const float2 im = __fadd2_rn(make_float2(biased_byte_to_float_bits(il, i), biased_byte_to_float_bits(ih, i)), bias);
+    float2 re = __fadd2_rn(make_float2(biased_byte_to_float_bits(rl, i), biased_byte_to_float_bits(rh, i)), bias);
+    float2 im = __fadd2_rn(make_float2(biased_byte_to_float_bits(il, i), biased_byte_to_float_bits(ih, i)), bias);
+    if (ph) {
+      const float4 p = __ldg(ph + i);
+      const float2 pr = make_float2(p.x, p.y), pi = make_float2(p.z, p.w);
+      const float2 r2 = __ffma2_rn(re, pr, neg2(__fmul2_rn(im, pi)));
+      im = __ffma2_rn(re, pi, __fmul2_rn(im, pr));
+      re = r2;
+    }
     e[i] = make_float4(re.x, re.y, im.x, im.y);
   }
+}
+
+// The untransposed input order [T][C][A][Np] with two polarisations: 8 consecutive
+// bytes hold (a0 X, a0 Y, a1 X, a1 Y | a2 X, a2 Y, a3 X, a3 Y); split them into the X and Y words.
+__device__ __forceinline__ void deinterleave_pols(uint32_t w0, uint32_t w1, uint32_t& wlo, uint32_t& whi) {
+  wlo = __byte_perm(w0, w1, 0x6420u);
+  whi = __byte_perm(w0, w1, 0x7531u);
 }
 
 // Compact form of the same unpack for large antenna counts: one 32-bit word per antenna holding

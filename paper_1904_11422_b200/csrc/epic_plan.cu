@@ -180,6 +180,10 @@ static int image_common(epic_plan* plan, const void* volt, int is_cf32, int n_t,
   ImageArgs a;
   a.volt = volt;
   a.is_cf32 = is_cf32;
+  a.native = plan->input_order == EPIC_ORDER_TCAP ? 1 : 0;
+  a.phasor = plan->d_phasor;
+  a.phasor_pair = plan->d_phasor_pair;
+  if (plan->d_phasor && (plan->ph_n_chan != n_chan || plan->ph_n_pol != n_pol)) return EPIC_ERR_ARG;
   a.n_t = n_t;
   a.n_chan = n_chan;
   a.n_pol = n_pol;
@@ -243,6 +247,10 @@ int epic_plan_create(epic_plan** out, int grid_n, int pad, int n_ant, const floa
   p->d_tiled = nullptr;
   p->tiled_ok = 0;
   p->d_auto = nullptr;
+  p->input_order = EPIC_ORDER_TCPA;
+  p->ph_n_chan = p->ph_n_pol = 0;
+  p->d_phasor = nullptr;
+  p->d_phasor_pair = nullptr;
   p->scratch_bytes = 0;
   p->scratch_limit = 0;
   int dev = 0;
@@ -291,6 +299,8 @@ int epic_plan_destroy(epic_plan* plan) {
   fused_plan_free(plan);
   tiled_plan_free(plan);
   autocorr_plan_free(plan);
+  if (plan->d_phasor) cudaFree(plan->d_phasor);
+  if (plan->d_phasor_pair) cudaFree(plan->d_phasor_pair);
   if (plan->d_scratch) cudaFree(plan->d_scratch);
   if (plan->d_blob) cudaFree(plan->d_blob);
   delete plan;
@@ -305,6 +315,48 @@ int epic_plan_set_products(epic_plan* plan, int n_products) {
   if (!plan) return EPIC_ERR_ARG;
   if (n_products != 0 && n_products != 1 && n_products != 2 && n_products != 4) return EPIC_ERR_RANGE;
   plan->n_products_req = n_products;
+  return EPIC_OK;
+}
+
+int epic_plan_set_input_order(epic_plan* plan, int order) {
+  if (!plan || (order != EPIC_ORDER_TCPA && order != EPIC_ORDER_TCAP)) return EPIC_ERR_ARG;
+  plan->input_order = order;
+  return EPIC_OK;
+}
+
+int epic_plan_set_delay_phasors(epic_plan* plan, int n_chan, int n_pol, const float* phasors) {
+  if (!plan) return EPIC_ERR_ARG;
+  EPIC_CUDA_TRY(cudaDeviceSynchronize());  // earlier calls may still read the old table
+  if (plan->d_phasor) cudaFree(plan->d_phasor);
+  if (plan->d_phasor_pair) cudaFree(plan->d_phasor_pair);
+  plan->d_phasor = nullptr;
+  plan->d_phasor_pair = nullptr;
+  plan->ph_n_chan = plan->ph_n_pol = 0;
+  if (!phasors) return EPIC_OK;
+  if (n_chan < 1 || (n_pol != 1 && n_pol != 2)) return EPIC_ERR_ARG;
+  const size_t A = (size_t)plan->n_ant, n = (size_t)n_chan * n_pol * A;
+  std::vector<float4> pair((size_t)n_chan * A);
+  for (int c = 0; c < n_chan; ++c)
+    for (size_t a = 0; a < A; ++a) {
+      const float* lo = phasors + (((size_t)c * n_pol + 0) * A + a) * 2;
+      const float* hi = phasors + (((size_t)c * n_pol + (n_pol - 1)) * A + a) * 2;
+      pair[(size_t)c * A + a] = make_float4(lo[0], hi[0], lo[1], hi[1]);
+    }
+  cudaError_t ce = cudaMalloc(&plan->d_phasor, n * sizeof(float2));
+  if (ce == cudaSuccess) ce = cudaMalloc(&plan->d_phasor_pair, pair.size() * sizeof(float4));
+  if (ce == cudaSuccess) ce = cudaMemcpy(plan->d_phasor, phasors, n * sizeof(float2), cudaMemcpyHostToDevice);
+  if (ce == cudaSuccess)
+    ce = cudaMemcpy(plan->d_phasor_pair, pair.data(), pair.size() * sizeof(float4), cudaMemcpyHostToDevice);
+  if (ce != cudaSuccess) {
+    set_cuda_error(ce);
+    if (plan->d_phasor) cudaFree(plan->d_phasor);
+    if (plan->d_phasor_pair) cudaFree(plan->d_phasor_pair);
+    plan->d_phasor = nullptr;
+    plan->d_phasor_pair = nullptr;
+    return ce == cudaErrorMemoryAllocation ? EPIC_ERR_NOMEM : EPIC_ERR_CUDA;
+  }
+  plan->ph_n_chan = n_chan;
+  plan->ph_n_pol = n_pol;
   return EPIC_OK;
 }
 
@@ -348,6 +400,10 @@ int epic_autocorr_remove(epic_plan* plan, const void* voltages, int n_t, int n_c
   ImageArgs a;
   a.volt = voltages;
   a.is_cf32 = 0;
+  a.native = plan->input_order == EPIC_ORDER_TCAP ? 1 : 0;
+  a.phasor = plan->d_phasor;
+  a.phasor_pair = plan->d_phasor_pair;
+  if (plan->d_phasor && (plan->ph_n_chan != n_chan || plan->ph_n_pol != n_pol)) return EPIC_ERR_ARG;
   a.n_t = n_t;
   a.n_chan = n_chan;
   a.n_pol = n_pol;

@@ -54,6 +54,8 @@ struct TiledParams {
   int n_t, n_chan, n_pol, n_planes;
   int c0, p0, Cb, Tb;    // batch: channels [c0, c0+Cb) x pairs [p0, p0+Tb)
   int nbx, nby;          // prefold counts along x (row pass) and y (column pass)
+  int native;            // input order [T][C][A][Np] instead of [T][C][Np][A]
+  const float4* phasor;  // delay phasors, pair-packed [C][A], or nullptr
 };
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
@@ -92,6 +94,7 @@ __global__ void __launch_bounds__(NT_A) tiled_rows(TiledParams P) {
   const long long n_items = (long long)P.Cb * P.Tb * n_groups;
   const int item0 = (int)(n_items * blockIdx.x / gridDim.x), item1 = (int)(n_items * (blockIdx.x + 1) / gridDim.x);
   int fb_loaded = -1;
+  const float4* ph_c = nullptr;  // this frame's channel's delay phasors
   for (int i = tid; i < RG * N; i += NT_A) buf[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
   for (int item = item0; item < item1; ++item) {
     const int fb = item / n_groups, g = item - fb * n_groups;
@@ -104,10 +107,17 @@ __global__ void __launch_bounds__(NT_A) tiled_rows(TiledParams P) {
       const uint8_t* lo = P.volt + ((size_t)t_lo * P.n_chan + c) * row_bytes;
       const uint8_t* hi = P.volt + ((size_t)t_hi * P.n_chan + c) * row_bytes + (P.n_pol == 2 ? t.n_ant : 0);
       for (int q = tid; q < (t.n_ant >> 2); q += NT_A) {
-        const uint32_t wlo = t_lo < P.n_t ? __ldg(reinterpret_cast<const uint32_t*>(lo) + q) : 0u;
-        const uint32_t whi = t_hi < P.n_t ? __ldg(reinterpret_cast<const uint32_t*>(hi) + q) : 0u;
+        uint32_t wlo = 0u, whi = 0u;
+        if (P.native && P.n_pol == 2) {  // (a X, a Y) byte pairs
+          if (t_lo < P.n_t) deinterleave_pols(__ldg(reinterpret_cast<const uint32_t*>(lo) + 2 * q),
+                                              __ldg(reinterpret_cast<const uint32_t*>(lo) + 2 * q + 1), wlo, whi);
+        } else {
+          if (t_lo < P.n_t) wlo = __ldg(reinterpret_cast<const uint32_t*>(lo) + q);
+          if (t_hi < P.n_t) whi = __ldg(reinterpret_cast<const uint32_t*>(hi) + q);
+        }
         *reinterpret_cast<uint4*>(E + 4 * q) = unpack_words_b8(wlo, whi);
       }
+      ph_c = P.phasor ? P.phasor + (size_t)c * t.n_ant : nullptr;
     }
     __syncthreads();  // E and the zeroed row buffer (end of the previous item) are complete
     const int y0 = g * RG, rows = min(RG, t.R - y0);
@@ -132,7 +142,15 @@ __global__ void __launch_bounds__(NT_A) tiled_rows(TiledParams P) {
           for (int k = 0; k < 4; ++k) {
             if (e + k < e_end) {
               float2 vr, vi;
-              b8_to_pair(E[__float_as_uint(rec[k].z)], vr, vi);
+              const uint32_t ant = __float_as_uint(rec[k].z);
+              b8_to_pair(E[ant], vr, vi);
+              if (ph_c) {  // delay compensation (reading Q19)
+                const float4 pp = __ldg(ph_c + ant);
+                const float2 pr = make_float2(pp.x, pp.y), pi = make_float2(pp.z, pp.w);
+                const float2 r2 = __ffma2_rn(vr, pr, neg2(__fmul2_rn(vi, pi)));
+                vi = __ffma2_rn(vr, pi, __fmul2_rn(vi, pr));
+                vr = r2;
+              }
               if (DELTA) {
                 sr = __fadd2_rn(sr, vr); si = __fadd2_rn(si, vi);
               } else {
@@ -516,6 +534,8 @@ int tiled_image(epic_plan* p, const ImageArgs& a) {
   P.tw1 = tt->tw1;
   P.tw2 = tt->tw2;
   P.ent_rec = tt->ent_rec;
+  P.native = a.native;
+  P.phasor = a.phasor_pair;
   P.n_t = a.n_t;
   P.n_chan = a.n_chan;
   P.n_pol = a.n_pol;

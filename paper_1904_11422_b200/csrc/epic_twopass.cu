@@ -32,15 +32,20 @@ __device__ __forceinline__ float2 cmul(float2 a, float2 w) {
 // ---------------------------------------------------------------- S3: one cell of the gather
 // G[cell] = sum over the cell's (antenna, tap) list of W * E, in (antenna, tap) order
 // (PAPER.md:122-124).  v points at this frame-and-polarisation's antenna vector.
+// Antenna a's sample is v[a * a_stride] (a_stride = n_pol for the untransposed input order,
+// PAPER.md:120); `ph` (or nullptr) holds this channel-and-polarisation's delay phasors
+// (reading Q19).
 template <bool CF32>
-__device__ __forceinline__ float2 gather_cell(const DevTables& t, const CellRec c, const void* v) {
+__device__ __forceinline__ float2 gather_cell(const DevTables& t, const CellRec c, const void* v, int a_stride = 1,
+                                              const float2* __restrict__ ph = nullptr) {
   float2 s = make_float2(0.0f, 0.0f);
   for (uint32_t e = c.ent_begin; e < c.ent_begin + c.ent_count; ++e) {
     const int a = t.ent_ant[e];
     const float2 w = t.ent_tap[e];
     float2 E;
-    if (CF32) E = reinterpret_cast<const float2*>(v)[a];
-    else E = unpack_ci4(reinterpret_cast<const uint8_t*>(v)[a]);
+    if (CF32) E = reinterpret_cast<const float2*>(v)[(size_t)a * a_stride];
+    else E = unpack_ci4(reinterpret_cast<const uint8_t*>(v)[(size_t)a * a_stride]);
+    if (ph) E = cmul(E, ph[a]);
     s.x = fmaf(w.x, E.x, s.x);
     s.x = fmaf(-w.y, E.y, s.x);
     s.y = fmaf(w.x, E.y, s.y);
@@ -79,6 +84,8 @@ struct BatchGeom {
   int C, Np, A;       // call shape
   int RB;             // support rows per kernel-A block
   int W;              // image columns per kernel-B block
+  int native;         // input order [T][C][A][Np] instead of [T][C][Np][A]
+  const float2* phasor; // delay phasors [C][Np][A] or nullptr
 };
 
 // ---------------------------------------------------------------- kernel A
@@ -96,7 +103,10 @@ __global__ void __launch_bounds__(256) grid_rowfft(DevTables t, BatchGeom g, con
   const int cb = fb / g.Tb, tb = fb - cb * g.Tb;
   const int r0 = blockIdx.x * g.RB;
   const int rows = min(g.RB, t.R - r0);
-  const size_t vidx = (((size_t)(g.t0 + tb) * g.C + (g.c0 + cb)) * g.Np + pol) * (size_t)g.A;
+  const size_t vidx = ((size_t)(g.t0 + tb) * g.C + (g.c0 + cb)) * g.Np * (size_t)g.A +
+                      (g.native ? (size_t)pol : (size_t)pol * g.A);
+  const int a_stride = g.native ? g.Np : 1;
+  const float2* ph = g.phasor ? g.phasor + ((size_t)(g.c0 + cb) * g.Np + pol) * g.A : nullptr;
   const void* v = CF32 ? (const void*)(reinterpret_cast<const float2*>(volt) + vidx)
                        : (const void*)(reinterpret_cast<const uint8_t*>(volt) + vidx);
   for (int i = tid; i < (N >> 1); i += 256) tw[i] = t.twiddle[i];
@@ -105,7 +115,7 @@ __global__ void __launch_bounds__(256) grid_rowfft(DevTables t, BatchGeom g, con
   const uint32_t cbeg = t.row_ptr[r0], cend = t.row_ptr[r0 + rows];
   for (uint32_t ci = cbeg + tid; ci < cend; ci += 256) {
     const CellRec c = t.cells[ci];
-    bx[(c.y - r0) * N + c.x] = gather_cell<CF32>(t, c, v);
+    bx[(c.y - r0) * N + c.x] = gather_cell<CF32>(t, c, v, a_stride, ph);
   }
   __syncthreads();
   float2* x = bx;
@@ -229,6 +239,8 @@ int twopass_image(epic_plan* p, const ImageArgs& a) {
   g.C = a.n_chan;
   g.Np = a.n_pol;
   g.A = p->n_ant;
+  g.native = a.native;
+  g.phasor = a.phasor;
   g.RB = std::max(1, std::min(R, 2048 / N));
   g.W = std::max(1, std::min(N, 2048 / N));
   const int strips = N / g.W;

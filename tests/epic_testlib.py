@@ -10,7 +10,7 @@ TOL = 1e-4  # BASELINE.json north_star: max |gpu - oracle| / image peak, fp32 pa
 
 
 def run_gpu(wl, volt=None, path=None, calls=1, n_products=None, return_plan_info=False, scratch_limit=None,
-            autocorr=False):
+            autocorr=False, native=False, phasors=None):
     import torch
     import paper_1904_11422_b200 as epic
 
@@ -22,6 +22,10 @@ def run_gpu(wl, volt=None, path=None, calls=1, n_products=None, return_plan_info
             plan.set_path(path)
         if scratch_limit is not None:
             plan.set_scratch_limit(scratch_limit)
+        if native:  # v is then [T][C][A][Np](,2)
+            plan.set_input_order(epic.EPIC_ORDER_TCAP)
+        if phasors is not None:
+            plan.set_delay_phasors(phasors)
         planes = plan.n_planes(wl.n_pol)
         out = torch.zeros((wl.n_chan, planes, wl.N, wl.N), dtype=torch.float32, device="cuda")
         dv = torch.from_numpy(v).cuda()

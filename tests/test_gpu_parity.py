@@ -269,6 +269,62 @@ def test_autocorr_removal_matches_oracle(wl, calls):
     assert_parity(gpu, ref, what=f"{wl.name} autocorr removed")
 
 
+# ------------------------------------------------------------------ upstream steps folded into the load
+UPSTREAM = [
+    (make_config(2, n_chan=3, n_t=21), None),                                     # fused, delta
+    (make_config(3, n_chan=2, n_t=13), None),                                     # fused, taps, TMEM variant
+    (make_config(4, n_chan=2, n_t=4), None),                                      # tiled
+    (make_custom(grid_n=32, pad=2, n_ant=40, n_pol=1, kernel_k=3, n_chan=3, n_t=9, layout="disc"), None),
+    (make_custom(grid_n=8, pad=2, n_ant=30, n_pol=2, kernel_k=3, n_chan=2, n_t=5, layout="wrap"), None),  # two-pass
+    (make_custom(grid_n=16, pad=2, n_ant=9, n_pol=2, kernel_k=1, n_chan=2, n_t=3, input_kind="cf32"), None),
+    (make_config(2, n_chan=2, n_t=8), 1),                                         # fused plan forced two-pass
+]
+
+
+@pytest.mark.parametrize("wl,path", UPSTREAM, ids=lambda v: v.name if hasattr(v, "name") else str(v))
+@pytest.mark.parametrize("mode", ["native", "phasors", "both"])
+def test_input_order_and_delay_phasors(wl, path, mode):
+    """[T][C][A][Np] input order and per-(channel, pol, antenna) delay phasors
+     through every kernel family, against the oracle with the same options; the
+    autocorrelation removal honours both."""
+    v = wl.voltages()
+    native = mode in ("native", "both")
+    rng = np.random.default_rng(5)
+    ph = None
+    if mode in ("phasors", "both"):
+        ph = (np.exp(2j * np.pi * rng.random((wl.n_chan, wl.n_pol, wl.n_ant))) *
+              rng.uniform(0.8, 1.25, (wl.n_chan, wl.n_pol, wl.n_ant))).astype(np.complex64)
+    vin = np.ascontiguousarray(np.swapaxes(v, 2, 3)) if native else v
+    kw = dict(order="TCAP" if native else "TCPA", delay_phasors=ph)
+    gpu = run_gpu(wl, volt=vin, path=path, native=native, phasors=ph)
+    ref = orc.epic_image(vin, wl.input_kind, wl.ant_uv, wl.taps, wl.grid_n, wl.pad, wl.n_products,
+                         kernel_k=wl.kernel_k, **kw)
+    assert_parity(gpu, ref, what=f"{wl.name} {mode}")
+    if wl.input_kind == "ci4":
+        gpu2 = run_gpu(wl, volt=vin, path=path, native=native, phasors=ph, autocorr=True)
+        ref2 = ref - orc.autocorr_image(vin, wl.input_kind, wl.ant_uv, wl.taps, wl.grid_n, wl.pad, wl.n_products,
+                                        kernel_k=wl.kernel_k, **kw)
+        assert_parity(gpu2, ref2, what=f"{wl.name} {mode} autocorr removed")
+
+
+def test_delay_phasor_shape_is_checked():
+    epic = _epic()
+    import torch
+    wl = make_config(2, n_chan=2, n_t=4)
+    with epic.Plan(wl.grid_n, wl.pad, wl.ant_uv) as plan:
+        plan.set_products(2)
+        plan.set_delay_phasors(np.ones((3, 2, 256), dtype=np.complex64))   # table for 3 channels
+        out = torch.zeros((2, 2, 128, 128), dtype=torch.float32, device="cuda")
+        dv = torch.from_numpy(wl.voltages()).cuda()
+        with pytest.raises(epic.EpicError):
+            plan.image(dv, 4, 2, 2, out)                                   # call with 2 channels
+        plan.set_delay_phasors(None)
+        plan.image(dv, 4, 2, 2, out)
+        torch.cuda.synchronize()
+        with pytest.raises(epic.EpicError):
+            plan.set_input_order(7)
+
+
 def test_calls_accumulate_into_out_accum():
     wl = make_config(2, n_chan=2, n_t=30)
     one = run_gpu(wl, calls=1)

@@ -399,3 +399,55 @@ def test_pixel_values_equal_the_imaged_pixels(wl):
                            kernel_k=wl.kernel_k)
     for i, (m, l) in enumerate(pix):
         assert np.abs(got[:, :, i] - img[:, :, m, l]).max() <= 1e-10 * np.abs(img).max()
+
+
+# ------------------------------------------------------------------ upstream steps: input order, delay phasors
+def test_untransposed_order_axes_hand_case():
+    """[T][C][A][Np] order: one sample at antenna 3, polarisation 0 must light up
+    XX only, flat, with value |E|^2; the same bytes read as [T][C][Np][A] would be (pol 1, antenna 2)."""
+    n_ant = 4
+    uv = np.array([[1, 1], [2, 5], [6, 3], [4, 4]], dtype=np.float32)
+    v = np.zeros((1, 1, n_ant, 2), dtype=np.uint8)          # TCAP
+    v[0, 0, 3, 0] = pack_ci4(3, -4)
+    img = orc.epic_image(v, "ci4", uv, None, 8, 1, 2, order="TCAP")
+    assert np.allclose(img[0, 0], 25.0) and np.all(img[0, 1] == 0.0)
+    wrong = orc.epic_image(v.reshape(1, 1, 2, n_ant), "ci4", uv, None, 8, 1, 2)   # same bytes, other order
+    assert np.all(wrong[0, 0] == 0.0) and np.allclose(wrong[0, 1], 25.0)
+
+
+def test_delay_phasors_closed_forms():
+    """Q19: (i) a global phase changes nothing; (ii) a phase psi on pol X only rotates
+    XY by exp(i psi) and leaves XX, YY; (iii) |d| = 2 on every antenna of pol Y scales YY by 4."""
+    wl = make_custom(grid_n=8, pad=2, n_ant=12, n_pol=2, kernel_k=3, n_chan=2, n_t=4, n_products=4)
+    v = wl.voltages()
+    args = (v, "ci4", wl.ant_uv, wl.taps, 8, 2, 4)
+    base = orc.epic_image(*args, kernel_k=3)
+    one = np.ones((2, 2, 12), dtype=np.complex128)
+    assert np.allclose(orc.epic_image(*args, kernel_k=3, delay_phasors=one * np.exp(0.7j)), base, rtol=1e-12, atol=1e-9)
+    psi = 0.9
+    d = one.copy(); d[:, 0, :] = np.exp(1j * psi)
+    got = orc.epic_image(*args, kernel_k=3, delay_phasors=d)
+    xy0 = base[:, 2] + 1j * base[:, 3]
+    assert np.allclose(got[:, :2], base[:, :2]) and np.allclose(got[:, 2] + 1j * got[:, 3], xy0 * np.exp(1j * psi))
+    d = one.copy(); d[:, 1, :] = 2.0
+    got = orc.epic_image(*args, kernel_k=3, delay_phasors=d)
+    assert np.allclose(got[:, 0], base[:, 0]) and np.allclose(got[:, 1], 4.0 * base[:, 1])
+
+
+def test_delay_compensation_restores_a_point_source():
+    """Per-antenna cable phases phi_a scramble a plane wave; the conjugate phasors bring the peak
+    back to the predicted pixel with the full coherent height A^2 |s|^2 T (check (c) with delays)."""
+    rng = np.random.default_rng(21)
+    n, n_ant, t_n = 16, 20, 3
+    cells = rng.choice(n * n, size=n_ant, replace=False)
+    uv = np.stack([cells % n, cells // n], axis=1).astype(np.float32)
+    kl, km = 5, 11
+    phi = rng.uniform(0, 2 * np.pi, n_ant)
+    e = np.exp(-2j * np.pi * (uv[:, 0] * kl + uv[:, 1] * km) / n) * np.exp(1j * phi)     # [A]
+    v = np.zeros((t_n, 1, 1, n_ant, 2), dtype=np.float32)
+    v[..., 0], v[..., 1] = e.real, e.imag
+    raw = orc.epic_image(v, "cf32", uv, None, n, 1, 1)
+    fixed = orc.epic_image(v, "cf32", uv, None, n, 1, 1, delay_phasors=np.exp(-1j * phi)[None, None, :])
+    assert np.unravel_index(np.argmax(fixed[0, 0]), (n, n)) == (km, kl)
+    assert fixed[0, 0, km, kl] == pytest.approx(t_n * n_ant ** 2, rel=1e-5)   # cf32 inputs
+    assert raw[0, 0].max() < 0.5 * fixed[0, 0, km, kl]
