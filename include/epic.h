@@ -80,7 +80,8 @@ EPIC_API int epic_plan_destroy(epic_plan* plan);
  * two need n_pol == 2.  Checked against n_pol at epic_image time.  0 restores the default. */
 EPIC_API int epic_plan_set_products(epic_plan* plan, int n_products);
 
-/* Select the kernel family (testing / benchmarking).  EPIC_ERR_RANGE if the plan cannot use it. */
+/* Select the kernel family (testing / benchmarking): an epic_path value.  EPIC_ERR_RANGE if the plan
+ * cannot use it (FUSED: occupied cells within 32x32 and N = 64 or 128; TILED: N = 256 or 512). */
 EPIC_API int epic_plan_set_path(epic_plan* plan, int path);
 
 /* Tuning: bytes of the plan's scratch (the intermediate H of the tiled / two-pass paths) one batch may

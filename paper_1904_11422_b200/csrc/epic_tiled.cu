@@ -1,7 +1,8 @@
 // Tiled two-pass EPIC path for large planes (N = 256, 512; any support): the packed (f32x2)
 // transform core of epic_packed.cuh, with the row-transformed plane H passed between two kernels
-// through an L2-resident scratch (BASELINE.json north_star (3): "two-pass L2-resident FFT only
-// when the grid exceeds shared memory").  PAPER.md:122-126 steps S1..S6.
+// through the plan's scratch (BASELINE.json north_star (3): a two-pass FFT only when the grid
+// exceeds shared memory; the scratch is 1 GiB by default, epic_plan_set_scratch_limit caps a
+// batch so that H stays resident in the 126 MB L2).  PAPER.md:122-126 steps S1..S6.
 //
 //   kernel A  tiled_rows   S1 unpack the frame's voltages -> E (shared), S3 gather-gridding of a
 //                          group of occupied rows, S4 along x -> H[frame][y][l] (float4 pairs)
