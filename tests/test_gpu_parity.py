@@ -325,6 +325,53 @@ def test_delay_phasor_shape_is_checked():
             plan.set_input_order(7)
 
 
+# ------------------------------------------------------------------ randomised plans, every path the plan allows
+def _random_case(seed):
+    rng = np.random.default_rng(1000 + seed)
+    N = int(rng.choice([64, 128, 128, 256, 512]))
+    pad = int(rng.choice([1, 2, 4]))
+    grid_n = N // pad
+    n_pol = int(rng.choice([1, 2, 2]))
+    K = int(rng.choice([1, 3, 3, 5, 7]))
+    layout = str(rng.choice(["disc", "uniform", "wrap", "tight"]))
+    n_ant = 4 * int(rng.integers(1, 60))
+    n_chan, n_t = int(rng.integers(1, 6)), int(rng.integers(1, 26 if N <= 256 else 7))
+    n_products = 1 if n_pol == 1 else int(rng.choice([2, 4]))
+    uv = None
+    if layout == "tight":  # everything inside a box the fused kernel can take, at a random offset (may wrap)
+        side = int(rng.integers(1, 33 - (K - 1)))
+        off = rng.integers(-N, N, 2)
+        uv = (off + rng.uniform(0, max(side - 1, 0.01), (n_ant, 2))).astype(np.float32)
+    wl = make_custom(grid_n=grid_n, pad=pad, n_ant=n_ant, n_pol=n_pol, kernel_k=K, n_chan=n_chan, n_t=n_t,
+                     n_products=n_products, layout="uniform" if uv is not None else layout, seed=seed, ant_uv=uv)
+    return wl, rng
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_random_plans_all_paths(seed):
+    """Random shapes, layouts (incl. boxes that wrap around the plane edge), kernel sizes, input order
+    and delay phasors: every kernel family the plan supports against the oracle."""
+    epic = _epic()
+    wl, rng = _random_case(seed)
+    v = wl.voltages()
+    native = bool(rng.integers(0, 2))
+    ph = None
+    if rng.integers(0, 2):
+        ph = np.exp(2j * np.pi * rng.random((wl.n_chan, wl.n_pol, wl.n_ant))).astype(np.complex64)
+    vin = np.ascontiguousarray(np.swapaxes(v, 2, 3)) if native else v
+    ref = orc.epic_image(vin, wl.input_kind, wl.ant_uv, wl.taps, wl.grid_n, wl.pad, wl.n_products,
+                         kernel_k=wl.kernel_k, order="TCAP" if native else "TCPA", delay_phasors=ph)
+    with epic.Plan(wl.grid_n, wl.pad, wl.ant_uv, wl.taps, wl.kernel_k) as plan:
+        plan.set_products(wl.n_products)
+        auto = plan.path(wl.n_pol)
+    tried = []
+    for path in sorted({1, auto}):
+        gpu = run_gpu(wl, volt=vin, path=path, native=native, phasors=ph, calls=int(rng.integers(1, 3)))
+        assert_parity(gpu, ref, what=f"seed {seed} {wl.name} path={path}")
+        tried.append(path)
+    assert 1 in tried
+
+
 def test_calls_accumulate_into_out_accum():
     wl = make_config(2, n_chan=2, n_t=30)
     one = run_gpu(wl, calls=1)
