@@ -23,6 +23,7 @@ on small planes and the fast one is used for large ones.
 
 Readings of the paper where it is silent:
 Q1 high nibble real / low nibble imaginary, two's complement; Q4 nearest cell = floor(x+0.5);
+Q15 antenna coordinates (and taps) may differ per channel: cell = lambda_c / 2 (PAPER.md:122);
 Q6 cells wrap modulo N; Q8 +2 pi i (inverse transform); Q9 unnormalised; Q10 natural order,
 zenith at [0][0]; Q11 XY = A_X conj(A_Y); Q12 plain sum over time; Q14 plane order
 {XX} | {XX,YY} | {XX,YY,ReXY,ImXY,ReYX,ImYX}; Q19 delay compensation = one complex multiplier per
@@ -34,7 +35,9 @@ linearity; S4 library inverse FFT vs the literal sum, impulse -> plane wave, zer
 invariant; S5/S6 one- and two-antenna closed forms, YX = conj(XY); whole path: (a) FX
 equivalence with brute-force direct-Fourier imaging of all antenna pairs, (b) Parseval,
 (c) plane-wave source peaks at the predicted pixel with height A^2; autocorr_image:
-image minus it equals brute-force imaging of the pairs a != b, one antenna -> exactly the image.
+image minus it equals brute-force imaging of the pairs a != b, one antenna -> exactly the image;
+per-channel layouts: brute-force FX imaging with each channel's own cells, two-antenna fringe whose
+period follows the channel, one sky direction -> one pixel in every channel.
 Parity unpinned: only the nibble-order *convention* (Q1) and anything LWA-instrument specific
 (no instrument data exists here); every function below has at least one pin.
 """
@@ -127,6 +130,18 @@ def taps_to_complex(taps: Optional[np.ndarray], n_ant: int, kernel_k: int) -> np
     return t[..., 0] + 1j * t[..., 1]
 
 
+def channel_layout(ant_uv: np.ndarray, taps: Optional[np.ndarray], c: int):
+    """(ant_uv [A][2], taps [A][K][K][2] or None) of channel c.  The grid spacing is tied to "the
+    wavelength of the channel", so an antenna's coordinates in cell units, and with
+    them its sub-cell offset and taps, differ from channel to channel: ``ant_uv`` [C][A][2] and
+    ``taps`` [C][A][K][K][2] carry one layout per channel (reading Q15); arrays without
+    the leading axis are the one layout every channel shares."""
+    uv = np.asarray(ant_uv)
+    if uv.ndim == 3:
+        return uv[c], (None if taps is None else np.asarray(taps)[c])
+    return uv, taps
+
+
 # ------------------------------------------------------------------ S3: gridding
 def grid_frames(e: np.ndarray, cells: np.ndarray, w: np.ndarray, n: int) -> np.ndarray:
     """Convolve-and-grid (W * E' of Eq. 4-5).
@@ -211,7 +226,8 @@ def epic_image(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Option
     """Accumulated polarised images, float64 [C'][planes][N][N] (C' = len(channels) or C).
 
     voltages: ci4 uint8 [T][C][Np][A] or cf32 float32 [T][C][Np][A][2] (PAPER.md:120 order
-    [Time, Channel, Polarisation, Antenna]).  mode "definition" uses the literal double sum
+    [Time, Channel, Polarisation, Antenna]).  ant_uv / taps may carry a leading channel axis
+    (``channel_layout``).  mode "definition" uses the literal double sum
     for S4, "fast" the library inverse FFT.  ``channels`` restricts the work to some channels
     (used for sampled parity at full size; channels are independent).
     """
@@ -219,14 +235,15 @@ def epic_image(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Option
     t_n, c_n = voltages.shape[:2]
     n_pol, n_ant = (voltages.shape[3], voltages.shape[2]) if order == "TCAP" else voltages.shape[2:4]
     ch = list(range(c_n)) if channels is None else list(channels)
-    cells = tap_cells(ant_uv, kernel_k, n)
-    w = taps_to_complex(taps, n_ant, kernel_k)
     xform = idft2_definition if mode == "definition" else idft2_fast
     pl = n_planes(n_pol, n_products)
     acc = np.zeros((len(ch), pl, n, n), dtype=np.float64)
     if frames_per_batch is None:
         frames_per_batch = max(1, min(t_n, (1 << 21) // (n * n * n_pol)))
     for ci, c in enumerate(ch):
+        uv_c, taps_c = channel_layout(ant_uv, taps, c)
+        cells = tap_cells(uv_c, kernel_k, n)                 # S2
+        w = taps_to_complex(taps_c, n_ant, kernel_k)
         for t0 in range(0, t_n, frames_per_batch):
             e = channel_voltages(voltages, kind, c, t0, t0 + frames_per_batch, order, delay_phasors)  # [F][Np][A]
             f = e.shape[0]
@@ -253,16 +270,24 @@ def autocorr_image(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Op
     t_n, c_n = voltages.shape[:2]
     n_pol, n_ant = (voltages.shape[3], voltages.shape[2]) if order == "TCAP" else voltages.shape[2:4]
     ch = list(range(c_n)) if channels is None else list(channels)
-    cells = tap_cells(ant_uv, kernel_k, n)
-    w = taps_to_complex(taps, n_ant, kernel_k)
-    beam = np.empty((n_ant, n, n), dtype=np.float64)  # |What_a|^2
-    for a in range(n_ant):
-        one = np.zeros((1, n_ant), dtype=np.complex128)
-        one[0, a] = 1.0
-        beam[a] = np.abs(idft2_fast(grid_frames(one, cells, w, n))[0]) ** 2
+
+    def beams(uv_c, taps_c):
+        cells = tap_cells(uv_c, kernel_k, n)
+        w = taps_to_complex(taps_c, n_ant, kernel_k)
+        b = np.empty((n_ant, n, n), dtype=np.float64)  # |What_a|^2
+        for a in range(n_ant):
+            one = np.zeros((1, n_ant), dtype=np.complex128)
+            one[0, a] = 1.0
+            b[a] = np.abs(idft2_fast(grid_frames(one, cells, w, n))[0]) ** 2
+        return b
+
+    per_channel = np.asarray(ant_uv).ndim == 3
+    beam = None if per_channel else beams(ant_uv, taps)
     pl = n_planes(n_pol, n_products)
     out = np.zeros((len(ch), pl, n, n), dtype=np.float64)
     for ci, c in enumerate(ch):
+        if per_channel:
+            beam = beams(*channel_layout(ant_uv, taps, c))
         e = channel_voltages(voltages, kind, c, 0, None, order, delay_phasors)  # [T][Np][A]
         vxx = (np.abs(e[:, 0]) ** 2).sum(axis=0)       # [A]
         out[ci, 0] = np.tensordot(vxx, beam, axes=1)
@@ -294,16 +319,17 @@ def pixel_values(voltages: np.ndarray, kind: str, ant_uv: np.ndarray, taps: Opti
     t_n, c_n = voltages.shape[:2]
     n_pol, n_ant = (voltages.shape[3], voltages.shape[2]) if order == "TCAP" else voltages.shape[2:4]
     ch = list(range(c_n)) if channels is None else list(channels)
-    cells = tap_cells(ant_uv, kernel_k, n)          # [A][K][K] flat y*N + x
-    w = taps_to_complex(taps, n_ant, kernel_k)      # [A][K][K]
-    cy, cx = cells // n, cells % n
     pl = n_planes(n_pol, n_products)
     out = np.zeros((len(ch), pl, len(pixels)), dtype=np.float64)
-    for pi, (m, l) in enumerate(pixels):
-        phase = np.exp(1j * TWO_PI * ((cx * l + cy * m) % n) / n)
-        u = (w * phase).sum(axis=(1, 2))            # [A]: response of antenna a at this pixel
-        for ci, c in enumerate(ch):
-            e = channel_voltages(voltages, kind, c, 0, None, order, delay_phasors)   # [T][Np][A]
+    for ci, c in enumerate(ch):
+        uv_c, taps_c = channel_layout(ant_uv, taps, c)
+        cells = tap_cells(uv_c, kernel_k, n)            # [A][K][K] flat y*N + x
+        w = taps_to_complex(taps_c, n_ant, kernel_k)    # [A][K][K]
+        cy, cx = cells // n, cells % n
+        e = channel_voltages(voltages, kind, c, 0, None, order, delay_phasors)   # [T][Np][A]
+        for pi, (m, l) in enumerate(pixels):
+            phase = np.exp(1j * TWO_PI * ((cx * l + cy * m) % n) / n)
+            u = (w * phase).sum(axis=(1, 2))            # [A]: response of antenna a at this pixel
             a = e @ u                                        # [T][Np]
             out[ci, 0, pi] = (np.abs(a[:, 0]) ** 2).sum()
             if n_pol == 2:

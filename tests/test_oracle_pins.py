@@ -9,7 +9,7 @@ import numpy as np
 import pytest
 
 from oracle import epic_oracle as orc
-from workloads import make_config, make_custom, pack_ci4
+from workloads import make_config, make_custom, make_per_channel, pack_ci4
 
 RNG = np.random.default_rng(20190411)
 
@@ -451,3 +451,87 @@ def test_delay_compensation_restores_a_point_source():
     assert np.unravel_index(np.argmax(fixed[0, 0]), (n, n)) == (km, kl)
     assert fixed[0, 0, km, kl] == pytest.approx(t_n * n_ant ** 2, rel=1e-5)   # cf32 inputs
     assert raw[0, 0].max() < 0.5 * fixed[0, 0, km, kl]
+
+
+# ------------------------------------------------------------------ per-channel layouts (reading Q15)
+def _rand_ci4(*shape):
+    r = np.random.default_rng(321)
+    return pack_ci4(r.integers(-8, 8, shape), r.integers(-8, 8, shape))
+
+
+def test_per_channel_cells_brute_force_fx_imaging():
+    """Each channel imaged by brute-force FX (all antenna pairs, Eq. 1-2) with THAT channel's cells:
+    the cell spacing follows the channel's wavelength."""
+    n, a_n, c_n, t_n = 16, 5, 3, 4
+    pos = np.array([[-3.2, 1.1], [2.6, -2.2], [0.4, 3.3], [-1.7, -3.6], [3.9, 0.2]])  # cells of channel 0
+    scale = np.array([1.0, 1.31, 1.77])                      # nu_c / nu_0
+    uv = (8.0 + pos[None] * scale[:, None, None]).astype(np.float32)
+    v = _rand_ci4(t_n, c_n, 1, a_n)
+    img = orc.epic_image(v, "ci4", uv, None, 8, 2, 1)
+    e = orc.unpack_ci4(v)
+    seen = set()
+    for c in range(c_n):
+        cells = np.array([[math.floor(float(x) + 0.5) for x in row] for row in uv[c]])   # typed out here
+        seen.add(tuple(cells.ravel()))
+        fx = _fx_direct_image(e[:, c, 0, :], cells, n)
+        np.testing.assert_allclose(img[c, 0], fx.real, atol=1e-9 * np.abs(fx).max())
+    assert len(seen) == c_n  # the three channels really use three different sets of cells
+
+
+def test_per_channel_two_antenna_fringe_follows_the_channel():
+    n = 32
+    uv = np.array([[[4, 6], [9, 6]], [[4, 6], [14, 6]]], np.float32)  # separation 5 cells, then 10
+    v = np.zeros((1, 2, 1, 2, 2), np.float32)
+    v[..., 0] = 1.0
+    img = orc.epic_image(v, "cf32", uv, None, 16, 2, 1)
+    l = np.arange(n)
+    for c, d in enumerate([5, 10]):
+        np.testing.assert_allclose(img[c, 0], np.broadcast_to(2 + 2 * np.cos(2 * np.pi * d * l / n), (n, n)), atol=1e-10)
+
+
+def test_per_channel_one_sky_direction_is_one_pixel_in_every_channel():
+    """On lambda_c/2 cells a plane wave from direction cosine l0 has phase -pi u_c l0 at an antenna
+    whose coordinate is u_c cells, so it lands on pixel l0 N / 2 in every channel."""
+    n, kl, km = 32, 5, -3
+    base = np.array([[1, 2], [3, -1], [-2, 2], [0, -3], [2, 1], [-3, -2]], np.float64)
+    uv = np.stack([8 + base, 8 + 3 * base]).astype(np.float32)       # nu_1 = 3 nu_0: integer cells in both
+    e = np.exp(-2j * np.pi * ((uv[..., 0] - 8) * kl + (uv[..., 1] - 8) * km) / n)   # [C][A]
+    v = np.zeros((1, 2, 1, 6, 2), np.float32)
+    v[0, :, 0, :, 0], v[0, :, 0, :, 1] = e.real, e.imag
+    img = orc.epic_image(v, "cf32", uv, None, 16, 2, 1)
+    for c in range(2):
+        pk = np.unravel_index(np.argmax(img[c, 0]), (n, n))
+        assert pk == (km % n, kl % n)
+        assert img[c, 0][pk] == pytest.approx(36.0, rel=1e-5)
+
+
+def test_per_channel_taps_single_antenna_closed_form():
+    """One antenna: XX = sum_t |E|^2 |sum_d W_c[d] exp(2 pi i (dx l + dy m)/N)|^2 with the channel's taps."""
+    n = 16
+    r = np.random.default_rng(5)
+    taps = r.standard_normal((2, 1, 3, 3, 2)).astype(np.float32)
+    uv = np.array([[[3.2, 4.9]], [[6.6, 2.1]]], np.float32)
+    v = _rand_ci4(3, 2, 1, 1)
+    img = orc.epic_image(v, "ci4", uv, taps, 8, 2, 1, kernel_k=3)
+    p = (np.abs(orc.unpack_ci4(v)) ** 2).sum(axis=0)[:, 0, 0]          # [C]
+    m, l = np.meshgrid(np.arange(n), np.arange(n), indexing="ij")
+    for c in range(2):
+        w = taps[c, 0, ..., 0].astype(np.float64) + 1j * taps[c, 0, ..., 1]
+        beam = sum(w[dy + 1, dx + 1] * np.exp(2j * np.pi * (dx * l + dy * m) / n) for dy in (-1, 0, 1) for dx in (-1, 0, 1))
+        np.testing.assert_allclose(img[c, 0], p[c] * np.abs(beam) ** 2, rtol=1e-10, atol=1e-9)
+
+
+def test_per_channel_autocorr_and_pixel_values_follow_the_channel():
+    wl = make_per_channel(grid_n=8, pad=2, n_ant=7, n_pol=2, kernel_k=3, n_chan=3, n_t=5,
+                          f0_hz=30e6, df_hz=12e6, diameter_m=25.0)
+    v = wl.voltages()
+    img = orc.epic_image(v, "ci4", wl.ant_uv, wl.taps, 8, 2, 4, kernel_k=3)
+    px = [(0, 0), (3, 11), (15, 2)]
+    pv = orc.pixel_values(v, "ci4", wl.ant_uv, wl.taps, 8, 2, 4, px, kernel_k=3)
+    for i, (m, l) in enumerate(px):
+        np.testing.assert_allclose(pv[:, :, i], img[:, :, m, l], atol=1e-9 * np.abs(img).max())
+    # one antenna: the image IS its autocorrelation term, channel by channel
+    ac = orc.autocorr_image(v[..., :1], "ci4", wl.ant_uv[:, :1], wl.taps[:, :1], 8, 2, 4, kernel_k=3)
+    one = orc.epic_image(v[..., :1], "ci4", wl.ant_uv[:, :1], wl.taps[:, :1], 8, 2, 4, kernel_k=3)
+    np.testing.assert_allclose(ac, one, atol=1e-9 * np.abs(one).max())
+    assert np.abs(one[0, 0] - one[2, 0] * one[0, 0].sum() / one[2, 0].sum()).max() > 1e-3 * one[0, 0].max()

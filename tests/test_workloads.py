@@ -68,3 +68,18 @@ def test_custom_wrap_layout_has_out_of_range_positions():
     wl = make_custom(grid_n=8, pad=2, n_ant=30, n_pol=1, kernel_k=3, n_chan=1, n_t=2, layout="wrap")
     assert wl.ant_uv.min() < 0 and wl.ant_uv.max() > 16
     assert wl.voltages().shape == (2, 1, 1, 30)
+
+
+def test_tophat_taps_cover_fractions_and_per_channel_scaling():
+    from workloads import make_per_channel, tophat_taps
+    t = tophat_taps(np.array([[3.0, 4.0]], np.float32), 3, 1.5)[0, ..., 0]
+    np.testing.assert_allclose(t, np.outer([1 / 6, 2 / 3, 1 / 6], [1 / 6, 2 / 3, 1 / 6]), rtol=1e-6)
+    t = tophat_taps(np.array([[3.25, 4.0]], np.float32), 3, 1.0)[0, ..., 0]      # shifted a quarter cell in x
+    np.testing.assert_allclose(t, np.outer([0, 1, 0], [0, 0.75, 0.25]), atol=1e-7)
+    wl = make_per_channel(grid_n=32, pad=2, n_ant=12, n_pol=2, kernel_k=3, n_chan=4, n_t=2,
+                          f0_hz=40e6, df_hz=10e6, diameter_m=60.0)
+    assert wl.ant_uv.shape == (4, 12, 2) and wl.taps.shape == (4, 12, 3, 3, 2)
+    off = wl.ant_uv.astype(np.float64) - 16.0
+    np.testing.assert_allclose(off[3], off[0] * 70.0 / 40.0, rtol=1e-5, atol=1e-5)   # cells ~ 1/lambda
+    np.testing.assert_allclose(np.abs(wl.taps[..., 0] + 1j * wl.taps[..., 1]).sum(axis=(-2, -1)), 1.0, rtol=1e-5)
+    assert wl.voltages().shape == (2, 4, 2, 12)

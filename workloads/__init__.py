@@ -12,7 +12,9 @@ from .configs import (  # noqa: F401
     Workload,
     make_config,
     make_custom,
+    make_per_channel,
     pack_ci4,
     gaussian_taps,
+    tophat_taps,
     CONFIG_NAMES,
 )

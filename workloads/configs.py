@@ -63,6 +63,35 @@ def gaussian_taps(ant_uv: np.ndarray, k: int, sigma: float, phase: np.ndarray) -
     return out
 
 
+def tophat_taps(ant_uv: np.ndarray, k: int, width_cells, phase: Optional[np.ndarray] = None) -> np.ndarray:
+    """Square top-hat illumination of side ``width_cells`` centred on each antenna's true position
+    ("a simple square top-hat function with 3-meter extent"), sampled as the fraction
+    of each cell [j-1/2, j+1/2) it covers, separable in x and y, normalised to sum 1, times an
+    optional per-antenna phase.  float32 [..., A, K, K, 2] for ant_uv [..., A, 2]; width_cells is a
+    scalar or broadcasts over the leading (channel) axis."""
+    uv = np.asarray(ant_uv, dtype=np.float32).astype(np.float64)
+    f = uv - _round_half_up(uv)
+    h = (k - 1) // 2
+    d = np.arange(-h, h + 1, dtype=np.float64)
+    half = 0.5 * np.asarray(width_cells, dtype=np.float64)
+    half = half.reshape(half.shape + (1,) * (uv.ndim - 1 - half.ndim) + (1,)) if half.ndim else half
+
+    def cover(frac):  # [..., A] -> [..., A, K]: overlap of [frac-half, frac+half] with [d-1/2, d+1/2]
+        lo = np.maximum(frac[..., None] - half, d - 0.5)
+        hi = np.minimum(frac[..., None] + half, d + 0.5)
+        return np.clip(hi - lo, 0.0, None)
+
+    w = cover(f[..., 1])[..., :, None] * cover(f[..., 0])[..., None, :]
+    w = w / w.sum(axis=(-2, -1), keepdims=True)
+    wc = w.astype(np.complex128)
+    if phase is not None:
+        wc = wc * np.exp(1j * np.asarray(phase, dtype=np.float64))[..., None, None]
+    out = np.empty(wc.shape + (2,), dtype=np.float32)
+    out[..., 0] = wc.real
+    out[..., 1] = wc.imag
+    return out
+
+
 @dataclass
 class Workload:
     name: str
@@ -77,8 +106,8 @@ class Workload:
     n_t: int
     input_kind: str  # "cf32" | "ci4"
     n_products: int  # 1 (XX), 2 (XX,YY) or 4 (XX,YY,XY,YX)
-    ant_uv: np.ndarray  # float32 [A][2] = (u, v) in cell units
-    taps: Optional[np.ndarray] = None  # float32 [A][K][K][2] or None (delta kernel)
+    ant_uv: np.ndarray  # float32 [A][2] = (u, v) in cell units, or [C][A][2]: one layout per channel
+    taps: Optional[np.ndarray] = None  # float32 [A][K][K][2] ([C][A][K][K][2]) or None (delta kernel)
     tap_phase: Optional[np.ndarray] = None  # float64 [A]; voltages carry e^{-i phase}
     noise_sigma: float = 2.0
     sources: List[dict] = field(default_factory=list)  # {"l_pix","m_pix","var"}
@@ -105,17 +134,19 @@ class Workload:
 
     # ---- voltages -----------------------------------------------------------------
     def _source_steer(self) -> Optional[np.ndarray]:
-        """complex128 [n_src][A]: geometric phase of a plane wave from pixel (l_pix, m_pix),
-        times the per-antenna instrumental phase e^{-i phi_a} that the taps undo."""
+        """complex128 [n_src][A] ([C][n_src][A] for per-channel layouts): geometric phase of a
+        plane wave from pixel (l_pix, m_pix), times the per-antenna instrumental phase
+        e^{-i phi_a} that the taps undo.  On lambda_c/2 cells a direction is the same pixel in
+        every channel, so per-channel coordinates need no other change."""
         if not self.sources:
             return None
         uv = self.ant_uv.astype(np.float64)
         inst = np.exp(-1j * self.tap_phase) if self.tap_phase is not None else 1.0
         rows = []
         for s in self.sources:
-            ph = -2.0 * np.pi * (uv[:, 0] * s["l_pix"] + uv[:, 1] * s["m_pix"]) / self.N
+            ph = -2.0 * np.pi * (uv[..., 0] * s["l_pix"] + uv[..., 1] * s["m_pix"]) / self.N
             rows.append(np.exp(1j * ph) * inst)
-        return np.stack(rows)
+        return np.stack(rows, axis=-2)
 
     def voltage_block(self, block: int, n_rows: int) -> np.ndarray:
         """Time samples [block*50, block*50 + n_rows) as uint8 [n_rows][C][Np][A] (ci4) or
@@ -133,7 +164,7 @@ class Workload:
             wv = rw.standard_normal((_TIME_BLOCK, C, len(self.sources), 2))[:n_rows]
             amp = np.sqrt(np.array([s["var"] for s in self.sources]) / 2.0)
             wave = (wv[..., 0] + 1j * wv[..., 1]) * amp  # [t][C][n_src]
-            sig = np.einsum("tcs,sa->tca", wave, steer)  # same waveform in both pols
+            sig = np.einsum("tcs,csa->tca" if steer.ndim == 3 else "tcs,sa->tca", wave, steer)  # same waveform in both pols
             x[..., 0] += sig.real[:, :, None, :].astype(np.float32)
             x[..., 1] += sig.imag[:, :, None, :].astype(np.float32)
         q = np.clip(np.rint(x), -8, 7).astype(np.int8)
@@ -265,4 +296,33 @@ def make_custom(*, grid_n: int, pad: int, n_ant: int, n_pol: int, kernel_k: int,
     src = _draw_sources(s, n_sources, N, max(n_t, 1), n_ant, 2.0) if n_sources else []
     name = f"custom-{n_ant}ant-{N}x{N}-k{kernel_k}-p{n_pol}-{input_kind}-s{seed}"
     return Workload(name, 0, s, grid_n, pad, n_ant, n_pol, kernel_k, n_chan, n_t, input_kind,
+                    n_products, uv, taps, ph, 2.0, src)
+
+
+def make_per_channel(*, grid_n: int, pad: int, n_ant: int, n_pol: int, kernel_k: int, n_chan: int, n_t: int,
+                     f0_hz: float, df_hz: float, diameter_m: float = 100.0, tophat_m: float = 3.0,
+                     n_products: Optional[int] = None, n_sources: int = 0, seed: int = 7,
+                     layout_seed: Optional[int] = None) -> Workload:
+    """One layout per channel: antennas uniform in area in
+    a disc of ``diameter_m`` metres, channel c at f0 + c df with cell = lambda_c / 2, so
+    ant_uv[c] = grid_n/2 + position / cell_c; kernel_k = 1 is the delta kernel, otherwise the
+    ``tophat_m`` square top-hat sampled at each channel's cell size with a per-antenna phase."""
+    s = BASE_SEED + 2000 + seed
+    r = _rng(s if layout_seed is None else layout_seed, _S_POS)
+    rad = 0.5 * diameter_m * np.sqrt(r.random(n_ant))
+    th = 2.0 * np.pi * r.random(n_ant)
+    pos = np.stack([rad * np.cos(th), rad * np.sin(th)], axis=1)        # metres, [A][2]
+    freq = f0_hz + df_hz * np.arange(n_chan, dtype=np.float64)
+    cell_m = 299792458.0 / freq / 2.0                                     # [C]
+    uv = (grid_n / 2.0 + pos[None, :, :] / cell_m[:, None, None]).astype(np.float32)
+    if n_products is None:
+        n_products = 4 if n_pol == 2 else 1
+    taps = ph = None
+    if kernel_k > 1:
+        ph = _rng(s, _S_PHASE).uniform(0.0, 2.0 * np.pi, n_ant)
+        taps = tophat_taps(uv, kernel_k, tophat_m / cell_m, ph)
+    N = grid_n * pad
+    src = _draw_sources(s, n_sources, N, max(n_t, 1), n_ant, 2.0) if n_sources else []
+    name = f"perchan-{n_ant}ant-{N}x{N}-k{kernel_k}-p{n_pol}-{f0_hz / 1e6:g}MHz+{n_chan}x{df_hz / 1e3:g}kHz"
+    return Workload(name, 0, s, grid_n, pad, n_ant, n_pol, kernel_k, n_chan, n_t, "ci4",
                     n_products, uv, taps, ph, 2.0, src)
