@@ -25,7 +25,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from workloads import make_config  # noqa: E402
+from workloads import make_config, make_per_channel  # noqa: E402
 
 METRIC = "E-field frames/sec (chan x time gridded+FFT'd+accumulated)"
 UNIT = "frames/s"
@@ -51,6 +51,22 @@ def algorithmic_bytes_per_frame(wl) -> float:
     v = wl.n_pol * wl.n_ant * (8 if wl.input_kind == "cf32" else 1)
     img = 2.0 * wl.n_planes * wl.N * wl.N * 4 / wl.n_t
     return v + img
+
+
+def per_channel_variant(wl):
+    """The same shape as BASELINE.json's config (antennas, grid, channels x samples, products) with
+    one layout per channel: 25 kHz channels from 38 MHz, antennas uniform in a disc
+    that fills the same fraction of the aperture grid, delta kernel where the config has one and
+    the deployment's 3 m top-hat (3x3 cells at these wavelengths) where it has taps."""
+    if wl.index not in (2, 3, 4):
+        raise SystemExit("--per-channel-cells: configs 2, 3 and 4")
+    diameter_m = 100.0 * wl.grid_n / 64.0
+    pc = make_per_channel(grid_n=wl.grid_n, pad=wl.pad, n_ant=wl.n_ant, n_pol=wl.n_pol, kernel_k=min(wl.kernel_k, 3),
+                          n_chan=wl.n_chan, n_t=wl.n_t, n_products=wl.n_products, f0_hz=38e6, df_hz=25e3,
+                          diameter_m=diameter_m, layout_seed=wl.seed, seed=wl.index)
+    pc.name = f"{wl.name}+per-channel-cells"
+    pc.index = wl.index
+    return pc
 
 
 def max_over_ranks(values, device) -> list:
@@ -297,6 +313,7 @@ def run_epic(args, wl):
         "config": {"workload": wl.name, **{k: v for k, v in wl.describe().items() if k != "workload"},
                    "kernel_path": PATH_NAMES.get(path, str(path)),
                    "input_order": args.input_order, "delay_phasors": bool(args.delay_phasors),
+                   "layouts": int(wl.ant_uv.shape[0]) if wl.ant_uv.ndim == 3 else 1,
                    "support_box": list(support), "l2": f"flushed between iterations ({L2_FLUSH_BYTES >> 20} MiB write)",
                    "sharding": "independent replicas of the workload per GPU (channels are independent), no collective"},
         "roofline": {
@@ -338,8 +355,13 @@ def main():
     ap.add_argument("--delay-phasors", action="store_true", help="apply per-(channel, pol, antenna) delay phasors")
     ap.add_argument("--e2e-chunks", type=int, default=4, help="time chunks of the end-to-end leg (H2D overlapped)")
     ap.add_argument("--scratch-mib", type=int, default=0, help="cap the per-batch scratch (tiled / two-pass paths)")
+    ap.add_argument("--per-channel-cells", action="store_true",
+                    help="configs 2-4 with one antenna layout per 25 kHz channel (cell = lambda_c/2) and, for 3 and 4, "
+                         "the 3 m top-hat kernel (PAPER.md:122, 162-168)")
     args = ap.parse_args()
     wl = make_config(args.config, n_chan=args.n_chan, n_t=args.n_t, n_ant=args.n_ant)
+    if args.per_channel_cells:
+        wl = per_channel_variant(wl)
     if args.impl == "reference":
         run_reference(args, wl)
     else:

@@ -73,6 +73,24 @@ typedef enum epic_path {
 EPIC_API int epic_plan_create(epic_plan** out, int grid_n, int pad, int n_ant, const float* ant_uv,
                      const float* kernel_taps, int kernel_k);
 
+/* The same with ONE LAYOUT PER FREQUENCY CHANNEL.  The grid spacing is tied to "the wavelength of the
+ * channel" (lambda/2 at the deployment), so an antenna's coordinates
+ * in cell units -- and with them its nearest cell, its sub-cell offset and the taps of a kernel of
+ * fixed physical size such as the 3 m top-hat of PAPER.md:166 -- differ from channel to channel
+ * (reading Q15).
+ *   n_layout      number of channels the plan describes, >= 1.
+ *   ant_uv        float[n_layout][n_ant][2]; kernel_taps NULL or
+ *                 float[n_layout][n_ant][kernel_k][kernel_k][2]; otherwise as above.
+ * Channel c of every later call uses layout c: epic_image / epic_autocorr_remove then require
+ * n_chan == n_layout (EPIC_ERR_ARG otherwise); a plan with n_layout == 1 (what epic_plan_create
+ * makes) applies its one layout to any number of channels.  The occupied support box is the
+ * union over the layouts. */
+EPIC_API int epic_plan_create_per_channel(epic_plan** out, int grid_n, int pad, int n_ant, int n_layout,
+                                 const float* ant_uv, const float* kernel_taps, int kernel_k);
+
+/* Number of layouts of the plan (1 unless made by epic_plan_create_per_channel). */
+EPIC_API int epic_plan_get_n_layouts(const epic_plan* plan);
+
 /* Frees the plan's device tables and scratch.  NULL is a no-op.  Synchronises the device. */
 EPIC_API int epic_plan_destroy(epic_plan* plan);
 
@@ -134,7 +152,7 @@ EPIC_API int epic_autocorr_remove(epic_plan* plan, const void* voltages, int n_t
 /* Plan queries (host, synchronous). */
 EPIC_API int epic_plan_get_n(const epic_plan* plan);        /* N, or negative status */
 EPIC_API int epic_plan_get_n_planes(const epic_plan* plan, int n_pol); /* planes for current products */
-/* S2 result: cells_host HOST int[n_ant][kernel_k][kernel_k] = y*N + x of every tap. */
+/* S2 result: cells_host HOST int[n_layout][n_ant][kernel_k][kernel_k] = y*N + x of every tap. */
 EPIC_API int epic_plan_get_cells(const epic_plan* plan, int* cells_host);
 /* Circular bounding box of the occupied cells: HOST int[4] = {y0, x0, rows, cols}. */
 EPIC_API int epic_plan_get_support(const epic_plan* plan, int* box_host);
@@ -148,10 +166,14 @@ EPIC_API int epic_plan_last_launches(const epic_plan* plan);
  * epic_debug_grid:   S1+S3 for ONE frame through the plan's gather table.  voltages DEVICE as
  *                    in epic_image (is_cf32 != 0: as in epic_image_cf32) with n_t = n_chan = 1;
  *                    out_plane_dev DEVICE float[n_pol][N][N][2], overwritten, true
- *                    (un-relocated) cell positions. */
+ *                    (un-relocated) cell positions.  Uses layout 0;
+ * epic_debug_grid_layout: the same through layout `layout` (0 <= layout < n_layout) of a
+ *                    per-channel plan. */
 EPIC_API int epic_debug_unpack(const void* bytes_dev, long n, float* out_dev, epic_stream stream);
 EPIC_API int epic_debug_grid(epic_plan* plan, const void* voltages, int is_cf32, int n_pol,
                     float* out_plane_dev, epic_stream stream);
+EPIC_API int epic_debug_grid_layout(epic_plan* plan, int layout, const void* voltages, int is_cf32, int n_pol,
+                           float* out_plane_dev, epic_stream stream);
 
 /* FP32 FMA micro-benchmark used for the roofline denominator: runs `iters` dependent-chain
  * FFMA rounds on every SM and writes elapsed milliseconds and the flop count (HOST outputs).

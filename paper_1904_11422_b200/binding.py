@@ -22,6 +22,8 @@ EPIC_ORDER_TCPA, EPIC_ORDER_TCAP = 0, 1
 _vp, _i, _l = ctypes.c_void_p, ctypes.c_int, ctypes.c_long
 SYMBOLS = {
     "epic_plan_create": (_i, [ctypes.POINTER(_vp), _i, _i, _i, _vp, _vp, _i]),
+    "epic_plan_create_per_channel": (_i, [ctypes.POINTER(_vp), _i, _i, _i, _i, _vp, _vp, _i]),
+    "epic_plan_get_n_layouts": (_i, [_vp]),
     "epic_plan_destroy": (_i, [_vp]),
     "epic_plan_set_products": (_i, [_vp, _i]),
     "epic_plan_set_path": (_i, [_vp, _i]),
@@ -39,6 +41,7 @@ SYMBOLS = {
     "epic_plan_last_launches": (_i, [_vp]),
     "epic_debug_unpack": (_i, [_vp, _l, _vp, _vp]),
     "epic_debug_grid": (_i, [_vp, _vp, _i, _i, _vp, _vp]),
+    "epic_debug_grid_layout": (_i, [_vp, _i, _vp, _i, _i, _vp, _vp]),
     "epic_fp32_peak_probe": (_i, [_i, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_double)]),
     "epic_status_string": (ctypes.c_char_p, [_i]),
     "epic_last_cuda_error": (_i, []),
@@ -108,19 +111,25 @@ class Plan:
     def __init__(self, grid_n: int, pad: int, ant_uv: np.ndarray,
                  kernel_taps: Optional[np.ndarray] = None, kernel_k: int = 1):
         uv = np.ascontiguousarray(ant_uv, dtype=np.float32)
-        if uv.ndim != 2 or uv.shape[1] != 2:
-            raise ValueError("ant_uv must be [n_ant][2]")
+        if uv.ndim not in (2, 3) or uv.shape[-1] != 2:
+            raise ValueError("ant_uv must be [n_ant][2], or [n_chan][n_ant][2] for one layout per channel")
+        per_channel = uv.ndim == 3
         taps = None
         if kernel_taps is not None:
             taps = np.ascontiguousarray(kernel_taps, dtype=np.float32)
-            if taps.shape != (uv.shape[0], kernel_k, kernel_k, 2):
+            if taps.shape != uv.shape[:-1] + (kernel_k, kernel_k, 2):
                 raise ValueError(f"kernel_taps shape {taps.shape}")
         self._h = _vp()
-        self.n_ant = int(uv.shape[0])
+        self.n_ant = int(uv.shape[-2])
         self.kernel_k = int(kernel_k)
-        _check(lib().epic_plan_create(ctypes.byref(self._h), grid_n, pad, self.n_ant,
-                                      _ptr(uv), _ptr(taps), kernel_k), "epic_plan_create")
+        if per_channel:  # epic_plan_create_per_channel: channel c of every call uses ant_uv[c], kernel_taps[c]
+            _check(lib().epic_plan_create_per_channel(ctypes.byref(self._h), grid_n, pad, self.n_ant, int(uv.shape[0]),
+                                                      _ptr(uv), _ptr(taps), kernel_k), "epic_plan_create_per_channel")
+        else:
+            _check(lib().epic_plan_create(ctypes.byref(self._h), grid_n, pad, self.n_ant,
+                                          _ptr(uv), _ptr(taps), kernel_k), "epic_plan_create")
         self.N = lib().epic_plan_get_n(self._h)
+        self.n_layouts = _check(lib().epic_plan_get_n_layouts(self._h), "epic_plan_get_n_layouts")
 
     # -- lifetime
     def destroy(self) -> None:
@@ -178,9 +187,10 @@ class Plan:
         return _check(lib().epic_plan_last_launches(self._h), "epic_plan_last_launches")
 
     def cells(self) -> np.ndarray:
-        out = np.empty((self.n_ant, self.kernel_k, self.kernel_k), dtype=np.int32)
+        """int32 [n_ant][K][K] ([n_layouts][n_ant][K][K] for a per-channel plan): y*N + x of every tap."""
+        out = np.empty((self.n_layouts, self.n_ant, self.kernel_k, self.kernel_k), dtype=np.int32)
         _check(lib().epic_plan_get_cells(self._h, _ptr(out)), "epic_plan_get_cells")
-        return out
+        return out if self.n_layouts > 1 else out[0]
 
     def support(self) -> tuple:
         out = np.empty(4, dtype=np.int32)
@@ -204,14 +214,19 @@ class Plan:
         _check(lib().epic_autocorr_remove(self._h, _ptr(voltages), n_t, n_chan, n_pol, _ptr(out_accum),
                                           _stream(stream)), "epic_autocorr_remove")
 
-    def debug_grid(self, voltages, is_cf32: bool, n_pol: int, out_plane, stream=None) -> None:
-        _check(lib().epic_debug_grid(self._h, _ptr(voltages), int(bool(is_cf32)), n_pol,
-                                     _ptr(out_plane), _stream(stream)), "epic_debug_grid")
+    def debug_grid(self, voltages, is_cf32: bool, n_pol: int, out_plane, stream=None, layout: int = 0) -> None:
+        _check(lib().epic_debug_grid_layout(self._h, int(layout), _ptr(voltages), int(bool(is_cf32)), n_pol,
+                                            _ptr(out_plane), _stream(stream)), "epic_debug_grid_layout")
 
 
 # free functions with the names of include/epic.h
 def epic_plan_create(grid_n, pad, n_ant, ant_uv, kernel_taps, kernel_k=1) -> Plan:
     uv = np.asarray(ant_uv, dtype=np.float32).reshape(n_ant, 2)
+    return Plan(grid_n, pad, uv, kernel_taps, kernel_k)
+
+
+def epic_plan_create_per_channel(grid_n, pad, n_ant, n_layout, ant_uv, kernel_taps, kernel_k=1) -> Plan:
+    uv = np.asarray(ant_uv, dtype=np.float32).reshape(n_layout, n_ant, 2)
     return Plan(grid_n, pad, uv, kernel_taps, kernel_k)
 
 

@@ -104,9 +104,10 @@ __global__ void __launch_bounds__(256) autocorr_sum(const int4* __restrict__ pow
 // lags[(c * n_lag + q) * 6] = (Lxx.re, Lxx.im, Lyy.re, Lyy.im, Lxy.re, Lxy.im) = sum_a V_aa corr_a[q].
 // One warp per (channel, lag): lanes stride the antennas, then a fixed shuffle tree (deterministic).
 __global__ void __launch_bounds__(128) autocorr_lags(const float4* __restrict__ psum, const float2* __restrict__ corr,
-                                                     int n_ant, int n_lag, float* __restrict__ lags) {
+                                                     int n_ant, int n_lag, int corr_stride, float* __restrict__ lags) {
   const int c = blockIdx.x, q = blockIdx.y * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (q >= n_lag) return;
+  corr += (size_t)c * corr_stride * n_lag;  // this channel's layout (corr_stride = 0: one layout)
   float v[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   for (int a = lane; a < n_ant; a += 32) {
     const float4 p = __ldg(psum + (size_t)c * n_ant + a);
@@ -159,14 +160,14 @@ __global__ void __launch_bounds__(256) autocorr_subtract(const float* __restrict
 }
 
 struct AutoTables {
-  float2* corr;  // [A][(2K-1)^2]
+  float2* corr;  // [n_layout][A][(2K-1)^2]
 };
 
 }  // namespace
 
 int autocorr_plan_init(epic_plan* p, const float* taps) {
   p->d_auto = nullptr;
-  const int K = p->K, span = 2 * K - 1, n_lag = span * span, A = p->n_ant;
+  const int K = p->K, span = 2 * K - 1, n_lag = span * span, A = p->n_ant * p->n_layout;  // (layout, antenna) rows
   std::vector<float2> corr((size_t)A * n_lag);
   for (int a = 0; a < A; ++a)
     for (int ly = -(K - 1); ly <= K - 1; ++ly)
@@ -229,7 +230,8 @@ int autocorr_remove(epic_plan* p, const ImageArgs& a) {
     autocorr_power<1><<<dim3(CHUNKS, a.n_chan, gz), 128, 0, a.stream>>>(volt, a.n_t, a.n_chan, a.n_pol, A, a.native, power);
   }
   autocorr_sum<<<(a.n_chan * A + 255) / 256, 256, 0, a.stream>>>(power, a.n_chan, A, a.phasor_pair, psum);
-  autocorr_lags<<<dim3(a.n_chan, (n_lag + 3) / 4), 128, 0, a.stream>>>(psum, at->corr, A, n_lag, lags);
+  autocorr_lags<<<dim3(a.n_chan, (n_lag + 3) / 4), 128, 0, a.stream>>>(psum, at->corr, A, n_lag,
+                                                                         p->n_layout > 1 ? A : 0, lags);
   autocorr_subtract<<<dim3((N * N + 255) / 256, a.n_chan), 256, 0, a.stream>>>(lags, p->t.twiddle, N, K, a.n_planes,
                                                                               a.out);
   EPIC_CUDA_TRY(cudaGetLastError());

@@ -90,6 +90,7 @@ struct FusedParams {
   float* out;                // [C][planes][N][N]
   const uint2* cell_info;    // [32*32] cell slots sorted by entry count: x = (first entry << 8) | count,
                              // y = cell offset cy*HS + cx in a plane (0xFFFFFFFF: unused slot)
+  int cell_stride;           // 32*32 when every channel has its own table (reading Q15), else 0
   const uint16_t* ent_ant;   // gather entries, sorted by block cell
   const float2* ent_tap;
   const float4* tw;          // [2Q][TWV]: the TwSet of every residue rho
@@ -300,7 +301,9 @@ __device__ __forceinline__ void col_task_tmem(const float4* __restrict__ col, co
   tmem_wait_st();
 }
 
-template <int Q, int NPROD, bool DELTA, int NB>
+// PC: every channel has its own cell table (per-channel plans); a separate instantiation, because
+// making the cell records loop-variant costs the one-layout kernels 1-2 % (measured).
+template <int Q, int NPROD, bool DELTA, int NB, bool PC>
 __global__ void __launch_bounds__(64 * Q, 2)
 epic_fused_kernel(FusedParams P) {
   constexpr int NT = 64 * Q, N = 32 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
@@ -317,9 +320,11 @@ epic_fused_kernel(FusedParams P) {
   constexpr bool TMEM = NPROD == 4;        // accumulators in tensor memory
   constexpr int TCOLS = Q == 4 ? 128 : 64;  // 64 columns per warp; warps w and w + 4 share a lane quadrant
 
-  uint2 info[S * S / NT];
+  int unit = (int)(g0 / P.nb);
+  uint2 info[S * S / NT];  // this thread's cells of the current channel's layout
 #pragma unroll
-  for (int j = 0; j < S * S / NT; ++j) info[j] = __ldg(P.cell_info + tid + j * NT);
+  for (int j = 0; j < S * S / NT; ++j)
+    info[j] = __ldg(P.cell_info + (PC ? (size_t)(unit / Q) * (S * S) : (size_t)0) + tid + j * NT);
   for (int i = tid; i < F * PLANE; i += NT) gh[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);  // rows >= R stay zero
   for (int i = tid; i < 2 * Q * TWV; i += NT) tws[i] = __ldg(P.tw + i);
   __syncthreads();
@@ -397,7 +402,6 @@ epic_fused_kernel(FusedParams P) {
     }
   };
 
-  int unit = (int)(g0 / P.nb);
   int b = (int)(g0 - (long long)unit * P.nb);
   const int first_unit = unit;
   int seg_begin = b;  // first batch of the current unit done by this CTA
@@ -443,6 +447,13 @@ epic_fused_kernel(FusedParams P) {
       flush(unit, seg_begin == 0 && b == P.nb - 1, unit == first_unit ? 0 : 1);
       seg_begin = 0;
     }
+    if constexpr (PC) {
+      if (unit_n / Q != unit / Q && more) {  // the next channel's cells (gather_batch is done with these)
+#pragma unroll
+        for (int j = 0; j < S * S / NT; ++j)
+          info[j] = __ldg(P.cell_info + (size_t)(unit_n / Q) * (S * S) + tid + j * NT);
+      }
+    }
     unit = unit_n; b = b_n;
     __syncthreads();  // next batch's E is complete; gh is free
   }
@@ -459,11 +470,11 @@ size_t fused_smem_bytes(int n_ant) {
   return ((size_t)F * PLANE + (size_t)2 * Q * TWV + (size_t)F * n_ant) * sizeof(float4);
 }
 
-template <int Q, int NPROD, bool DELTA, int NB>
+template <int Q, int NPROD, bool DELTA, int NB, bool PC>
 int launch_fused(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
   constexpr int NT = 64 * Q;
   const size_t smem = fused_smem_bytes<Q>(P.n_ant);
-  auto kern = epic_fused_kernel<Q, NPROD, DELTA, NB>;
+  auto kern = epic_fused_kernel<Q, NPROD, DELTA, NB, PC>;
   if (smem > 48 * 1024)
     EPIC_CUDA_TRY(cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int per_sm = 0;
@@ -487,15 +498,17 @@ int launch_fused(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
 template <int Q, int NPROD, bool DELTA>
 int launch_fused_nb(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
   // elements y + 16 of a row/column are read only while y < NB (the rest of the block is empty)
-  if (std::max(p->R, p->Cc) <= 16 + 12) return launch_fused<Q, NPROD, DELTA, 12>(p, P, s);
-  return launch_fused<Q, NPROD, DELTA, 16>(p, P, s);
+  const bool pc = P.cell_stride != 0;
+  if (std::max(p->R, p->Cc) <= 16 + 12)
+    return pc ? launch_fused<Q, NPROD, DELTA, 12, true>(p, P, s) : launch_fused<Q, NPROD, DELTA, 12, false>(p, P, s);
+  return pc ? launch_fused<Q, NPROD, DELTA, 16, true>(p, P, s) : launch_fused<Q, NPROD, DELTA, 16, false>(p, P, s);
 }
 
 template <int Q>
 int launch_fused_q(const epic_plan* p, const FusedParams& P, int n_products, cudaStream_t s) {
   const bool delta = p->t.is_delta != 0;
 #ifdef EPIC_FUSED_DEV_ONE  // development builds: compile a single instantiation
-  if (Q == 4 && n_products == 2 && delta) return launch_fused<4, 2, true, 12>(p, P, s);
+  if (Q == 4 && n_products == 2 && delta) return launch_fused<4, 2, true, 12, false>(p, P, s);
   return EPIC_ERR_RANGE;
 #else
   switch (n_products) {
@@ -516,19 +529,25 @@ int fused_plan_init(epic_plan* p) {
   if (p->N % S != 0 || (Q != 2 && Q != 4)) return EPIC_OK;
   if (p->R > S || p->Cc > S) return EPIC_OK;
   if (p->h_ent_ant.size() >= ((size_t)1 << 24)) return EPIC_OK;
-  std::vector<uint32_t> dense((size_t)S * S, 0u);
-  for (const CellRec& c : p->h_cells) {
-    if (c.ent_count > 255u) return EPIC_OK;  // falls back to the two-pass path
-    dense[(size_t)c.y * S + c.x] = (c.ent_begin << 8) | c.ent_count;
-  }
-  // every cell of the R x 32 block (columns >= Cc are re-zeroed each batch: the row pass writes
-  // its output in place), sorted by entry count so that warps see uniform trip counts
+  // one table of S x S cell records per layout (channel c of a per-channel plan reads table c)
   std::vector<uint2> info;
-  for (int y = 0; y < p->R; ++y)
-    for (int x = 0; x < S; ++x) info.push_back(make_uint2(dense[(size_t)y * S + x], (uint32_t)(y * HS + x)));
-  std::stable_sort(info.begin(), info.end(),
-                   [](const uint2& l, const uint2& r) { return (l.x & 0xFFu) > (r.x & 0xFFu); });
-  info.resize((size_t)S * S, make_uint2(0u, 0xFFFFFFFFu));
+  for (int l = 0; l < p->n_layout; ++l) {
+    std::vector<uint32_t> dense((size_t)S * S, 0u);
+    for (uint32_t i = p->h_cell_off[l]; i < p->h_cell_off[l + 1]; ++i) {
+      const CellRec& c = p->h_cells[i];
+      if (c.ent_count > 255u) return EPIC_OK;  // falls back to the two-pass path
+      dense[(size_t)c.y * S + c.x] = (c.ent_begin << 8) | c.ent_count;
+    }
+    // every cell of the R x 32 block (columns >= Cc are re-zeroed each batch: the row pass writes
+    // its output in place), sorted by entry count so that warps see uniform trip counts
+    std::vector<uint2> li;
+    for (int y = 0; y < p->R; ++y)
+      for (int x = 0; x < S; ++x) li.push_back(make_uint2(dense[(size_t)y * S + x], (uint32_t)(y * HS + x)));
+    std::stable_sort(li.begin(), li.end(),
+                     [](const uint2& a, const uint2& b) { return (a.x & 0xFFu) > (b.x & 0xFFu); });
+    li.resize((size_t)S * S, make_uint2(0u, 0xFFFFFFFFu));
+    info.insert(info.end(), li.begin(), li.end());
+  }
   // TwSet of every residue rho = 0..2Q-1, from double (reading Q8: + sign): r = exp(2 pi i rho / N)
   std::vector<float4> tw((size_t)2 * Q * TWV);
   for (int rho = 0; rho < 2 * Q; ++rho) {
@@ -596,6 +615,7 @@ int fused_image(epic_plan* p, const ImageArgs& a) {
   P.volt = static_cast<const uint8_t*>(a.volt);
   P.out = a.out;
   P.cell_info = ft->cell_info;
+  P.cell_stride = p->n_layout > 1 ? S * S : 0;
   P.ent_ant = p->t.ent_ant;
   P.ent_tap = p->t.ent_tap;
   P.tw = ft->tw;

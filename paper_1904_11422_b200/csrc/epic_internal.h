@@ -17,14 +17,18 @@ struct CellRec {
 };
 
 struct DevTables {
-  const CellRec* cells;     // [n_cells], sorted by (y, x)
-  const uint32_t* row_ptr;  // [R + 1]: cells of support row y are [row_ptr[y], row_ptr[y+1])
+  // With n_layout > 1 (one antenna layout per channel, reading Q15) the tables of the
+  // layouts are concatenated: channel c's row pointers start at row_ptr + c * row_stride and hold
+  // indices into the common cells array, whose ent_begin index the common entry arrays.
+  const CellRec* cells;     // [n_cells], each layout's cells sorted by (y, x)
+  const uint32_t* row_ptr;  // [n_layout][R + 1]: cells of support row y are [row_ptr[y], row_ptr[y+1])
   const uint16_t* ent_ant;  // [n_ent] antenna index of each gather entry
   const float2* ent_tap;    // [n_ent] complex tap of each gather entry
   const float2* twiddle;    // [N/2]: exp(+2 pi i k / N), computed in double on the host
   int n_cells, n_ent;
   int N, logN, R, Cc, y0, x0; // support box: rows [y0, y0+R) mod N, cols [x0, x0+Cc) mod N
   int n_ant, is_delta;
+  int n_layout, row_stride; // row_stride = R + 1 when n_layout > 1, else 0 (every channel reads layout 0)
 };
 
 } // namespace epic
@@ -34,7 +38,8 @@ struct epic_plan {
   int n_products_req; // 0 = default
   int path_req;
   int last_launches;
-  std::vector<int> cells_host; // [n_ant][K][K] true cells y*N + x
+  int n_layout;                // antenna layouts: 1, or one per channel
+  std::vector<int> cells_host; // [n_layout][n_ant][K][K] true cells y*N + x
   int y0, x0, R, Cc;
   epic::DevTables t;           // device pointers
   void* d_blob;                // one allocation holding all tables
@@ -52,7 +57,8 @@ struct epic_plan {
   int tiled_ok;                // N is 256 or 512
   int n_sm;
   // host copies kept for the fused path's table builder
-  std::vector<epic::CellRec> h_cells;
+  std::vector<epic::CellRec> h_cells;   // all layouts, concatenated
+  std::vector<uint32_t> h_cell_off;     // [n_layout + 1]: layout l's cells are [h_cell_off[l], h_cell_off[l+1])
   std::vector<uint16_t> h_ent_ant;
   std::vector<float2> h_ent_tap;
 };
@@ -72,7 +78,7 @@ struct ImageArgs {
 
 // epic_twopass.cu
 int twopass_image(epic_plan* p, const ImageArgs& a);
-int debug_grid(epic_plan* p, const void* volt, int is_cf32, int n_pol, float* out, cudaStream_t s);
+int debug_grid(epic_plan* p, int layout, const void* volt, int is_cf32, int n_pol, float* out, cudaStream_t s);
 int debug_unpack(const void* bytes, long n, float* out, cudaStream_t s);
 int fp32_probe(int iters, float* ms, double* flops);
 

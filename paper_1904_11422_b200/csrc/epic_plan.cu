@@ -44,72 +44,84 @@ struct Entry {
   int ant, tap;  // tap = iy*K + ix
 };
 
-static int build_tables(epic_plan* p, const float* ant_uv, const float* taps) {
-  const int N = p->N, K = p->K, A = p->n_ant, h = (K - 1) / 2;
-  p->cells_host.resize((size_t)A * K * K);
+static int build_tables(epic_plan* p, const float* ant_uv_all, const float* taps_all) {
+  const int N = p->N, K = p->K, A = p->n_ant, h = (K - 1) / 2, L = p->n_layout;
+  const size_t per_layout = (size_t)A * K * K;
+  p->cells_host.resize((size_t)L * per_layout);
+  // S2 for every layout; the support box is the union of the occupied rows / columns
   std::vector<char> occ_y(N, 0), occ_x(N, 0);
-  for (int a = 0; a < A; ++a) {
-    // reading Q4: nearest cell = floor(double(u) + 0.5)
-    const long long cx = (long long)std::floor((double)ant_uv[2 * a + 0] + 0.5);
-    const long long cy = (long long)std::floor((double)ant_uv[2 * a + 1] + 0.5);
-    for (int iy = 0; iy < K; ++iy)
-      for (int ix = 0; ix < K; ++ix) {
-        const int y = pos_mod(cy + (iy - h), N); // reading Q6: wrap modulo N
-        const int x = pos_mod(cx + (ix - h), N);
-        p->cells_host[((size_t)a * K + iy) * K + ix] = y * N + x;
-        occ_y[y] = 1;
-        occ_x[x] = 1;
-      }
+  for (int l = 0; l < L; ++l) {
+    const float* ant_uv = ant_uv_all + (size_t)l * A * 2;
+    for (int a = 0; a < A; ++a) {
+      // reading Q4: nearest cell = floor(double(u) + 0.5)
+      const long long cx = (long long)std::floor((double)ant_uv[2 * a + 0] + 0.5);
+      const long long cy = (long long)std::floor((double)ant_uv[2 * a + 1] + 0.5);
+      for (int iy = 0; iy < K; ++iy)
+        for (int ix = 0; ix < K; ++ix) {
+          const int y = pos_mod(cy + (iy - h), N); // reading Q6: wrap modulo N
+          const int x = pos_mod(cx + (ix - h), N);
+          p->cells_host[l * per_layout + ((size_t)a * K + iy) * K + ix] = y * N + x;
+          occ_y[y] = 1;
+          occ_x[x] = 1;
+        }
+    }
   }
   circular_box(occ_y, N, &p->y0, &p->R);
   circular_box(occ_x, N, &p->x0, &p->Cc);
 
-  std::vector<Entry> ent((size_t)A * K * K);
-  for (int a = 0; a < A; ++a)
-    for (int k = 0; k < K * K; ++k) {
-      const int cell = p->cells_host[(size_t)a * K * K + k];
-      Entry e;
-      e.y = pos_mod(cell / N - p->y0, N);
-      e.x = pos_mod(cell % N - p->x0, N);
-      e.ant = a;
-      e.tap = k;
-      ent[(size_t)a * K * K + k] = e;
-    }
-  std::sort(ent.begin(), ent.end(), [](const Entry& l, const Entry& r) {
-    if (l.y != r.y) return l.y < r.y;
-    if (l.x != r.x) return l.x < r.x;
-    if (l.ant != r.ant) return l.ant < r.ant;
-    return l.tap < r.tap;
-  });
-
   p->h_cells.clear();
-  p->h_ent_ant.resize(ent.size());
-  p->h_ent_tap.resize(ent.size());
-  std::vector<uint32_t> row_ptr(p->R + 1, 0);
-  for (size_t i = 0; i < ent.size(); ++i) {
-    const Entry& e = ent[i];
-    if (p->h_cells.empty() || p->h_cells.back().y != e.y || p->h_cells.back().x != e.x) {
-      CellRec c;
-      c.y = (uint16_t)e.y;
-      c.x = (uint16_t)e.x;
-      c.ent_begin = (uint32_t)i;
-      c.ent_count = 0;
-      p->h_cells.push_back(c);
-      row_ptr[e.y + 1] += 1;
+  p->h_cell_off.assign(1, 0u);
+  p->h_ent_ant.resize((size_t)L * per_layout);
+  p->h_ent_tap.resize((size_t)L * per_layout);
+  std::vector<uint32_t> row_ptr((size_t)L * (p->R + 1), 0);
+  std::vector<Entry> ent(per_layout);
+  for (int l = 0; l < L; ++l) {
+    const float* taps = taps_all ? taps_all + l * per_layout * 2 : nullptr;
+    for (int a = 0; a < A; ++a)
+      for (int k = 0; k < K * K; ++k) {
+        const int cell = p->cells_host[l * per_layout + (size_t)a * K * K + k];
+        Entry e;
+        e.y = pos_mod(cell / N - p->y0, N);
+        e.x = pos_mod(cell % N - p->x0, N);
+        e.ant = a;
+        e.tap = k;
+        ent[(size_t)a * K * K + k] = e;
+      }
+    std::sort(ent.begin(), ent.end(), [](const Entry& l_, const Entry& r_) {
+      if (l_.y != r_.y) return l_.y < r_.y;
+      if (l_.x != r_.x) return l_.x < r_.x;
+      if (l_.ant != r_.ant) return l_.ant < r_.ant;
+      return l_.tap < r_.tap;
+    });
+    const size_t cell0 = p->h_cells.size(), ent0 = l * per_layout;
+    uint32_t* rp = &row_ptr[(size_t)l * (p->R + 1)];
+    for (size_t i = 0; i < ent.size(); ++i) {
+      const Entry& e = ent[i];
+      if (p->h_cells.size() == cell0 || p->h_cells.back().y != e.y || p->h_cells.back().x != e.x) {
+        CellRec c;
+        c.y = (uint16_t)e.y;
+        c.x = (uint16_t)e.x;
+        c.ent_begin = (uint32_t)(ent0 + i);
+        c.ent_count = 0;
+        p->h_cells.push_back(c);
+        rp[e.y + 1] += 1;
+      }
+      p->h_cells.back().ent_count += 1;
+      p->h_ent_ant[ent0 + i] = (uint16_t)e.ant;
+      float2 w;
+      if (taps) {
+        w.x = taps[((size_t)e.ant * K * K + e.tap) * 2 + 0];
+        w.y = taps[((size_t)e.ant * K * K + e.tap) * 2 + 1];
+      } else {
+        w.x = 1.0f;
+        w.y = 0.0f;
+      }
+      p->h_ent_tap[ent0 + i] = w;
     }
-    p->h_cells.back().ent_count += 1;
-    p->h_ent_ant[i] = (uint16_t)e.ant;
-    float2 w;
-    if (taps) {
-      w.x = taps[((size_t)e.ant * K * K + e.tap) * 2 + 0];
-      w.y = taps[((size_t)e.ant * K * K + e.tap) * 2 + 1];
-    } else {
-      w.x = 1.0f;
-      w.y = 0.0f;
-    }
-    p->h_ent_tap[i] = w;
+    rp[0] = (uint32_t)cell0;  // indices into the concatenated cells array
+    for (int y = 0; y < p->R; ++y) rp[y + 1] += rp[y];
+    p->h_cell_off.push_back((uint32_t)p->h_cells.size());
   }
-  for (int y = 0; y < p->R; ++y) row_ptr[y + 1] += row_ptr[y];
 
   std::vector<float2> tw(N / 2);
   for (int k = 0; k < N / 2; ++k) {
@@ -142,7 +154,7 @@ static int build_tables(epic_plan* p, const float* ant_uv, const float* taps) {
   t.twiddle = (const float2*)(d + o_tw);
   t.ent_ant = (const uint16_t*)(d + o_ant);
   t.n_cells = (int)p->h_cells.size();
-  t.n_ent = (int)ent.size();
+  t.n_ent = (int)p->h_ent_ant.size();
   t.N = N;
   t.logN = p->logN;
   t.R = p->R;
@@ -150,7 +162,9 @@ static int build_tables(epic_plan* p, const float* ant_uv, const float* taps) {
   t.y0 = p->y0;
   t.x0 = p->x0;
   t.n_ant = A;
-  t.is_delta = taps ? 0 : 1;
+  t.is_delta = taps_all ? 0 : 1;
+  t.n_layout = L;
+  t.row_stride = L > 1 ? p->R + 1 : 0;
   return EPIC_OK;
 }
 
@@ -175,6 +189,7 @@ static int image_common(epic_plan* plan, const void* volt, int is_cf32, int n_t,
   const int n_planes = planes_for(n_pol, n_products);
   if (n_planes < 0) return EPIC_ERR_RANGE;
   plan->last_launches = 0;
+  if (plan->n_layout > 1 && n_chan != plan->n_layout) return EPIC_ERR_ARG;  // channel c uses layout c
   if (n_t == 0 || n_chan == 0) return EPIC_OK;
   if (!volt || !out) return EPIC_ERR_ARG;
   ImageArgs a;
@@ -217,16 +232,22 @@ extern "C" {
 
 int epic_plan_create(epic_plan** out, int grid_n, int pad, int n_ant, const float* ant_uv,
                      const float* kernel_taps, int kernel_k) {
+  return epic_plan_create_per_channel(out, grid_n, pad, n_ant, 1, ant_uv, kernel_taps, kernel_k);
+}
+
+int epic_plan_create_per_channel(epic_plan** out, int grid_n, int pad, int n_ant, int n_layout,
+                                 const float* ant_uv, const float* kernel_taps, int kernel_k) {
   if (!out) return EPIC_ERR_ARG;
   *out = nullptr;
-  if (!ant_uv || grid_n < 1 || pad < 1) return EPIC_ERR_ARG;
+  if (!ant_uv || grid_n < 1 || pad < 1 || n_layout < 1) return EPIC_ERR_ARG;
   const long long Nll = (long long)grid_n * pad;
   if (Nll < 8 || Nll > 512 || (Nll & (Nll - 1)) != 0) return EPIC_ERR_ARG;
   if (kernel_k < 1 || kernel_k > 15 || (kernel_k % 2) == 0) return EPIC_ERR_ARG;
   if (!kernel_taps && kernel_k != 1) return EPIC_ERR_ARG;
   if (n_ant < 1) return EPIC_ERR_ARG;
   if (n_ant > 65535) return EPIC_ERR_RANGE;
-  for (int i = 0; i < 2 * n_ant; ++i)
+  if ((long long)n_layout * n_ant * kernel_k * kernel_k > (1LL << 30)) return EPIC_ERR_RANGE;
+  for (long long i = 0; i < 2LL * n_layout * n_ant; ++i)
     if (!std::isfinite(ant_uv[i]) || std::fabs(ant_uv[i]) > 1.0e9f) return EPIC_ERR_ARG;
   epic_plan* p = new (std::nothrow) epic_plan();
   if (!p) return EPIC_ERR_NOMEM;
@@ -236,6 +257,7 @@ int epic_plan_create(epic_plan** out, int grid_n, int pad, int n_ant, const floa
   p->logN = 0;
   while ((1 << p->logN) < p->N) ++p->logN;
   p->n_ant = n_ant;
+  p->n_layout = n_layout;
   p->K = kernel_k;
   p->n_products_req = 0;
   p->path_req = EPIC_PATH_AUTO;
@@ -395,6 +417,7 @@ int epic_autocorr_remove(epic_plan* plan, const void* voltages, int n_t, int n_c
   const int n_planes = planes_for(n_pol, n_products);
   if (n_planes < 0) return EPIC_ERR_RANGE;
   plan->last_launches = 0;
+  if (plan->n_layout > 1 && n_chan != plan->n_layout) return EPIC_ERR_ARG;
   if (n_t == 0 || n_chan == 0) return EPIC_OK;
   if (!voltages || !out_accum) return EPIC_ERR_ARG;
   ImageArgs a;
@@ -415,6 +438,8 @@ int epic_autocorr_remove(epic_plan* plan, const void* voltages, int n_t, int n_c
 }
 
 int epic_plan_get_n(const epic_plan* plan) { return plan ? plan->N : (int)EPIC_ERR_ARG; }
+
+int epic_plan_get_n_layouts(const epic_plan* plan) { return plan ? plan->n_layout : (int)EPIC_ERR_ARG; }
 
 int epic_plan_get_n_planes(const epic_plan* plan, int n_pol) {
   if (!plan) return EPIC_ERR_ARG;
@@ -457,11 +482,17 @@ int epic_debug_unpack(const void* bytes_dev, long n, float* out_dev, epic_stream
   return debug_unpack(bytes_dev, n, out_dev, (cudaStream_t)stream);
 }
 
+int epic_debug_grid_layout(epic_plan* plan, int layout, const void* voltages, int is_cf32, int n_pol,
+                           float* out_plane_dev, epic_stream stream) {
+  if (!plan || !voltages || !out_plane_dev) return EPIC_ERR_ARG;
+  if (layout < 0 || layout >= plan->n_layout) return EPIC_ERR_ARG;
+  if (n_pol != 1 && n_pol != 2) return EPIC_ERR_RANGE;
+  return debug_grid(plan, layout, voltages, is_cf32 ? 1 : 0, n_pol, out_plane_dev, (cudaStream_t)stream);
+}
+
 int epic_debug_grid(epic_plan* plan, const void* voltages, int is_cf32, int n_pol,
                     float* out_plane_dev, epic_stream stream) {
-  if (!plan || !voltages || !out_plane_dev) return EPIC_ERR_ARG;
-  if (n_pol != 1 && n_pol != 2) return EPIC_ERR_RANGE;
-  return debug_grid(plan, voltages, is_cf32 ? 1 : 0, n_pol, out_plane_dev, (cudaStream_t)stream);
+  return epic_debug_grid_layout(plan, 0, voltages, is_cf32, n_pol, out_plane_dev, stream);
 }
 
 int epic_fp32_peak_probe(int iters, float* ms_out, double* flops_out) {

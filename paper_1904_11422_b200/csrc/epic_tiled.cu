@@ -127,7 +127,8 @@ __global__ void __launch_bounds__(NT_A<J>) tiled_rows(TiledParams P) {
     const int y0 = g * RG, rows = min(RG, t.R - y0);
     // S3: gather-gridding of the group's cells, one thread per cell, sums in table order.
     // Four cell records, then four entry records, are in flight per thread (L2 latency).
-    const uint32_t cbeg = __ldg(t.row_ptr + y0), cend = __ldg(t.row_ptr + y0 + rows);
+    const uint32_t* rp = t.row_ptr + (size_t)(P.c0 + fb / P.Tb) * t.row_stride;  // this channel's layout
+    const uint32_t cbeg = __ldg(rp + y0), cend = __ldg(rp + y0 + rows);
     for (uint32_t base = cbeg + tid; base < cend; base += 4 * NT_A<J>) {
       CellRec cr[4];
 #pragma unroll

@@ -112,7 +112,8 @@ __global__ void __launch_bounds__(256) grid_rowfft(DevTables t, BatchGeom g, con
   for (int i = tid; i < (N >> 1); i += 256) tw[i] = t.twiddle[i];
   for (int i = tid; i < rows * N; i += 256) bx[i] = make_float2(0.0f, 0.0f);
   __syncthreads();
-  const uint32_t cbeg = t.row_ptr[r0], cend = t.row_ptr[r0 + rows];
+  const uint32_t* rp = t.row_ptr + (size_t)(g.c0 + cb) * t.row_stride;  // this channel's layout
+  const uint32_t cbeg = rp[r0], cend = rp[r0 + rows];
   for (uint32_t ci = cbeg + tid; ci < cend; ci += 256) {
     const CellRec c = t.cells[ci];
     bx[(c.y - r0) * N + c.x] = gather_cell<CF32>(t, c, v, a_stride, ph);
@@ -296,22 +297,25 @@ int debug_unpack(const void* bytes, long n, float* out, cudaStream_t s) {
 }
 
 template <bool CF32>
-__global__ void grid_plane_kernel(DevTables t, const void* volt, int n_pol, float2* __restrict__ out) {
+__global__ void grid_plane_kernel(DevTables t, int layout, const void* volt, int n_pol, float2* __restrict__ out) {
   const int pol = blockIdx.y;
+  const uint32_t* rp = t.row_ptr + (size_t)layout * (t.R + 1);
+  const int c_begin = rp[0], c_end = rp[t.R];
   const void* v = CF32 ? (const void*)(reinterpret_cast<const float2*>(volt) + (size_t)pol * t.n_ant)
                        : (const void*)(reinterpret_cast<const uint8_t*>(volt) + (size_t)pol * t.n_ant);
-  for (int ci = blockIdx.x * blockDim.x + threadIdx.x; ci < t.n_cells; ci += gridDim.x * blockDim.x) {
+  for (int ci = c_begin + blockIdx.x * blockDim.x + threadIdx.x; ci < c_end; ci += gridDim.x * blockDim.x) {
     const CellRec c = t.cells[ci];
     const int y = (c.y + t.y0) & (t.N - 1), x = (c.x + t.x0) & (t.N - 1);
     out[((size_t)pol * t.N + y) * t.N + x] = gather_cell<CF32>(t, c, v);
   }
 }
 
-int debug_grid(epic_plan* p, const void* volt, int is_cf32, int n_pol, float* out, cudaStream_t s) {
+int debug_grid(epic_plan* p, int layout, const void* volt, int is_cf32, int n_pol, float* out, cudaStream_t s) {
   EPIC_CUDA_TRY(cudaMemsetAsync(out, 0, (size_t)n_pol * p->N * p->N * sizeof(float2), s));
-  const dim3 grid((p->t.n_cells + 255) / 256, n_pol);
-  if (is_cf32) grid_plane_kernel<true><<<grid, 256, 0, s>>>(p->t, volt, n_pol, (float2*)out);
-  else grid_plane_kernel<false><<<grid, 256, 0, s>>>(p->t, volt, n_pol, (float2*)out);
+  const int n_cells = (int)(p->h_cell_off[layout + 1] - p->h_cell_off[layout]);
+  const dim3 grid((n_cells + 255) / 256, n_pol);
+  if (is_cf32) grid_plane_kernel<true><<<grid, 256, 0, s>>>(p->t, layout, volt, n_pol, (float2*)out);
+  else grid_plane_kernel<false><<<grid, 256, 0, s>>>(p->t, layout, volt, n_pol, (float2*)out);
   EPIC_CUDA_TRY(cudaGetLastError());
   return EPIC_OK;
 }

@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 
 from oracle import epic_oracle as orc
-from workloads import make_config, make_custom
+from workloads import make_config, make_custom, make_per_channel
 
 from epic_testlib import TOL, assert_parity, run_gpu, run_oracle
 
@@ -414,3 +414,106 @@ def test_point_source_peaks_at_predicted_pixel():
     src = wl.sources[0]
     m, l = np.unravel_index(np.argmax(gpu[0, 2]), gpu[0, 2].shape)
     assert (m, l) == (src["m_pix"], src["l_pix"])
+
+
+# ------------------------------------------------------------------ one antenna layout per channel (reading Q15)
+PER_CHANNEL = [
+    # (workload, paths): 1 two-pass, 2 fused, 3 tiled
+    (make_per_channel(grid_n=64, pad=2, n_ant=64, n_pol=2, kernel_k=1, n_chan=5, n_t=37, n_products=2,
+                      f0_hz=30e6, df_hz=4e6, diameter_m=100.0), [1, 2]),
+    (make_per_channel(grid_n=64, pad=2, n_ant=96, n_pol=2, kernel_k=3, n_chan=7, n_t=23, f0_hz=38e6, df_hz=2e6,
+                      diameter_m=80.0, n_sources=1), [1, 2]),
+    (make_per_channel(grid_n=32, pad=2, n_ant=48, n_pol=1, kernel_k=3, n_chan=4, n_t=30, f0_hz=20e6, df_hz=7e6,
+                      diameter_m=90.0), [1, 2]),
+    (make_per_channel(grid_n=128, pad=2, n_ant=200, n_pol=2, kernel_k=3, n_chan=3, n_t=9, f0_hz=40e6, df_hz=9e6,
+                      diameter_m=300.0), [1, 3]),
+    (make_per_channel(grid_n=256, pad=2, n_ant=300, n_pol=2, kernel_k=1, n_chan=2, n_t=5, n_products=2,
+                      f0_hz=50e6, df_hz=20e6, diameter_m=500.0), [1, 3]),
+    (make_per_channel(grid_n=12, pad=2, n_ant=20, n_pol=2, kernel_k=5, n_chan=3, n_t=6, f0_hz=30e6, df_hz=10e6,
+                      diameter_m=30.0), [1]),   # N = 24 is not a power of two -> rejected below
+]
+
+
+@pytest.mark.parametrize("wl,paths", PER_CHANNEL[:5], ids=lambda v: v.name if hasattr(v, "name") else str(v))
+def test_per_channel_layouts_all_paths(wl, paths):
+    """epic_plan_create_per_channel: channel c is gridded with ITS cells and taps (cell = lambda_c / 2,
+    PAPER.md:122; 3 m top-hat).  Every kernel family against the oracle, and AUTO
+    picks the fast one."""
+    epic = _epic()
+    assert wl.ant_uv.ndim == 3
+    with epic.Plan(wl.grid_n, wl.pad, wl.ant_uv, wl.taps, wl.kernel_k) as plan:
+        assert plan.n_layouts == wl.n_chan
+        plan.set_products(wl.n_products)
+        assert plan.path(wl.n_pol) == paths[-1]
+        cells = plan.cells()
+    assert np.array_equal(cells.astype(np.int64),
+                          np.stack([orc.tap_cells(wl.ant_uv[c], wl.kernel_k, wl.N) for c in range(wl.n_chan)]))
+    assert len({cells[c].tobytes() for c in range(wl.n_chan)}) == wl.n_chan   # the layouts do differ
+    v = wl.voltages()
+    ref = run_oracle(wl, volt=v)
+    for path in paths:
+        gpu = run_gpu(wl, volt=v, path=path, calls=2)
+        assert_parity(gpu, ref, what=f"{wl.name} path {path}")
+
+
+def test_per_channel_gridding_one_frame_per_layout():
+    import torch
+    epic = _epic()
+    wl = PER_CHANNEL[1][0]
+    v = wl.voltages()
+    with epic.Plan(wl.grid_n, wl.pad, wl.ant_uv, wl.taps, wl.kernel_k) as plan:
+        for c in range(wl.n_chan):
+            e = orc.voltages_to_complex(v[0, c], wl.input_kind)  # [Np][A]
+            ref = orc.grid_frames(e, orc.tap_cells(wl.ant_uv[c], 3, wl.N), orc.taps_to_complex(wl.taps[c], wl.n_ant, 3), wl.N)
+            out = torch.full((wl.n_pol, wl.N, wl.N, 2), 7.0, dtype=torch.float32, device="cuda")
+            plan.debug_grid(torch.from_numpy(np.ascontiguousarray(v[0, c])).cuda(), False, wl.n_pol, out, layout=c)
+            torch.cuda.synchronize()
+            got = out.cpu().numpy()
+            gc = got[..., 0].astype(np.float64) + 1j * got[..., 1]
+            assert np.abs(gc - ref).max() <= 2e-6 * max(1.0, np.abs(ref).max())
+
+
+def test_per_channel_plan_checks_its_arguments():
+    import torch
+    epic = _epic()
+    wl = PER_CHANNEL[0][0]
+    with epic.Plan(wl.grid_n, wl.pad, wl.ant_uv, wl.taps, wl.kernel_k) as plan:
+        plan.set_products(2)
+        out = torch.zeros((wl.n_chan, 2, wl.N, wl.N), dtype=torch.float32, device="cuda")
+        dv = torch.from_numpy(wl.voltages()).cuda()
+        with pytest.raises(epic.EpicError) as ei:       # channel c uses layout c: n_chan must match
+            plan.image(dv, 3, wl.n_chan - 1, wl.n_pol, out)
+        assert ei.value.status == epic.EPIC_ERR_ARG
+        with pytest.raises(epic.EpicError):
+            plan.debug_grid(dv, False, wl.n_pol, out, layout=wl.n_chan)
+        plan.image(dv, 0, wl.n_chan, wl.n_pol, out)     # empty call is still a no-op
+        assert float(out.abs().max()) == 0.0
+    bad = PER_CHANNEL[5][0]
+    with pytest.raises(epic.EpicError):
+        epic.Plan(bad.grid_n, bad.pad, bad.ant_uv, bad.taps, bad.kernel_k)
+
+
+@pytest.mark.parametrize("wl", [PER_CHANNEL[1][0], PER_CHANNEL[3][0]], ids=lambda w: w.name)
+def test_per_channel_autocorr_removal(wl):
+    v = wl.voltages()
+    gpu = run_gpu(wl, volt=v, autocorr=True)
+    ref = run_oracle(wl, volt=v) - orc.autocorr_image(v, wl.input_kind, wl.ant_uv, wl.taps, wl.grid_n, wl.pad,
+                                                      wl.n_products, kernel_k=wl.kernel_k)
+    assert_parity(gpu, ref, what=f"{wl.name} autocorr removed")
+
+
+def test_per_channel_full_size_lwa_band():
+    """The C2 workload with the paper's channelisation: 128 channels of 25 kHz from
+    38 MHz, each on its own lambda_c / 2 grid, 3 m top-hat taps, in the launch configuration
+    `bench.py --per-channel-cells` times (one call, AUTO = fused); sampled channels against the oracle."""
+    wl = make_per_channel(grid_n=64, pad=2, n_ant=256, n_pol=2, kernel_k=3, n_chan=128, n_t=1000, n_products=2,
+                          f0_hz=38e6, df_hz=25e3, diameter_m=100.0, layout_seed=1904114222)
+    v = wl.voltages()
+    gpu, info = run_gpu(wl, volt=v, return_plan_info=True)
+    assert info["path"] == 2 and info["launches"] == 2
+    channels = [0, 64, 127]
+    ref = run_oracle(wl, volt=v, channels=channels)
+    assert_parity(gpu[channels], ref, what=f"{wl.name} channels {channels}")
+    assert np.isfinite(gpu).all() and (gpu >= 0).all()
+    totals = gpu[:, 0].sum(axis=(1, 2))
+    assert totals.min() > 0.5 * totals.max()
