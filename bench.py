@@ -31,8 +31,9 @@ METRIC = "E-field frames/sec (chan x time gridded+FFT'd+accumulated)"
 UNIT = "frames/s"
 FP32_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # SMs x lanes x FMA x max clock
 L2_FLUSH_BYTES = 256 << 20
-PATH_NAMES = {1: "twopass", 2: "fused", 3: "tiled"}
-PATH_KERNELS = {1: "grid_rowfft+colfft_accum", 2: "epic_fused_kernel (+ epic_fused_fixup, <1 % of the step)", 3: "tiled_rows+tiled_cols"}
+PATH_NAMES = {1: "twopass", 2: "fused", 3: "tiled", 4: "tensor"}
+PATH_KERNELS = {1: "grid_rowfft+colfft_accum", 2: "epic_fused_kernel (+ epic_fused_fixup, <1 % of the step)", 3: "tiled_rows+tiled_cols",
+                4: "epic_tc_kernel (column transform as BF16x3 tcgen05.mma; + epic_fused_fixup)"}
 
 
 def algorithmic_flops_per_frame(wl) -> float:
@@ -199,7 +200,7 @@ def run_epic(args, wl):
     plan = epic.Plan(wl.grid_n, wl.pad, wl.ant_uv, wl.taps, wl.kernel_k)
     plan.set_products(wl.n_products)
     if args.path:
-        plan.set_path({"auto": 0, "twopass": 1, "fused": 2, "tiled": 3}[args.path])
+        plan.set_path({"auto": 0, "twopass": 1, "fused": 2, "tiled": 3, "tensor": 4}[args.path])
     if args.scratch_mib:
         plan.set_scratch_limit(args.scratch_mib << 20)
     if args.input_order == "tcap":
@@ -345,7 +346,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (1-based)")
     ap.add_argument("--impl", default="epic", choices=["epic", "reference"])
-    ap.add_argument("--path", default=None, choices=[None, "auto", "twopass", "fused", "tiled"])
+    ap.add_argument("--path", default=None, choices=[None, "auto", "twopass", "fused", "tiled", "tensor"])
     ap.add_argument("--n-chan", type=int, default=None)
     ap.add_argument("--n-t", type=int, default=None)
     ap.add_argument("--n-ant", type=int, default=None)

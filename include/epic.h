@@ -55,7 +55,10 @@ typedef enum epic_path {
   EPIC_PATH_AUTO = 0,
   EPIC_PATH_TWOPASS = 1, /* grid+row-FFT kernel -> L2-resident scratch -> column-FFT+products kernel */
   EPIC_PATH_FUSED = 2,   /* one kernel (+ a tiny ordered fix-up of split units), planes never leave the SM (occupied cells within 32x32, N = 64, 128) */
-  EPIC_PATH_TILED = 3    /* N = 256, 512: packed row kernel -> L2-resident scratch -> packed column kernel */
+  EPIC_PATH_TILED = 3,   /* N = 256, 512: packed row kernel -> L2-resident scratch -> packed column kernel */
+  EPIC_PATH_TENSOR = 4   /* the fused kernel with its column transform as a dense BF16x3 contraction on the
+                            tensor cores (tcgen05.mma); N = 128, two polarisations, one layout.  Never
+                            picked by AUTO: measured and reported beside the FP32 path */
 } epic_path;
 
 /* S2 + plan set-up ("gridded onto a 2D grid ... spacing < lambda/2"; illumination

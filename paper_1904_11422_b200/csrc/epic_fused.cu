@@ -38,6 +38,11 @@
 //   at the end of the unit's time range: one add per pixel into out_accum (directly, or through
 //   the partial-sum fix-up kernel when the unit's time range was split between two CTAs).
 #include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+#include <cuda_bf16.h>
 
 #include "epic_internal.h"
 #include "epic_packed.cuh"
@@ -242,7 +247,7 @@ __device__ __forceinline__ void add_pixel(float* __restrict__ px, size_t plane, 
 
 // Adds the parked partial sums of every unit whose time range was split between CTAs, in CTA
 // order.  One CTA per unit, same thread <-> pixel mapping as the main kernel.
-template <int Q, int NPROD>
+template <int Q, int NPROD, bool TC = false>
 __global__ void __launch_bounds__(64 * Q) epic_fused_fixup(FusedParams P, int main_grid) {
   constexpr int NT = 64 * Q, N = 32 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
   const int unit = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -253,7 +258,12 @@ __global__ void __launch_bounds__(64 * Q) epic_fused_fixup(FusedParams P, int ma
   const int rho = (warp >> 1) * 2 + (lane & 1);
   const int c = unit / Q, l2 = unit - c * Q;
   const size_t plane = (size_t)N * N;
-  float* o = P.out + (size_t)c * P.n_planes * plane + (Q * l1 + l2);
+  float* o = P.out + (size_t)c * P.n_planes * plane + (Q * l1 + l2) + (size_t)rho * N;
+  size_t kstride = (size_t)2 * Q * N;
+  if constexpr (TC) {  // tensor-core kernel: thread = (image row m, 16 columns l1), see epic_tc_kernel
+    o = P.out + (size_t)c * P.n_planes * plane + (size_t)((warp & 3) * 32 + lane) * N + Q * 16 * (warp >> 2) + l2;
+    kstride = Q;
+  }
   for (int k = 0; k < 16; ++k) {
     float v[NACC];
 #pragma unroll
@@ -264,7 +274,7 @@ __global__ void __launch_bounds__(64 * Q) epic_fused_fixup(FusedParams P, int ma
 #pragma unroll
       for (int q = 0; q < NACC; ++q) v[q] += part[(size_t)(q * 16 + k) * NT];
     }
-    add_pixel<NPROD>(o + (size_t)(2 * Q * k + rho) * N, plane, v);
+    add_pixel<NPROD>(o + k * kstride, plane, v);
   }
 }
 
@@ -460,9 +470,233 @@ epic_fused_kernel(FusedParams P) {
   if constexpr (TMEM) tmem_free_cta<TCOLS>(tbase, warp);
 }
 
+
+// ================================================================ tensor-core column pass
+// The column transform of a unit is a dense contraction: A[m][(f, pol, l1)] = sum_y F[m][y] H[y][(f, pol, l1)],
+// F[m][y] = exp(+2 pi i m y / N) (128 x 32), H = the row-pass output of the batch (32 x 256).  Here it
+// runs on the 5th-generation tensor cores (tcgen05.mma, BF16 in, FP32 accumulators in tensor memory)
+// instead of the pruned FFT: complex = 4 real products, and to hold the 1e-4 image tolerance every
+// operand is split hi + lo in BF16 (16 mantissa bits) with the lo x lo term dropped:
+//
+//   D_r = Fr Hr - Fi Hi,  D_i = Fi Hr + Fr Hi,  X Y ~ X_hi Y_hi + X_hi Y_lo + X_lo Y_hi
+//
+// = 24 MMAs of M 128 x N 256 x K 16 per batch (12 per accumulator; the minus sign is the
+// instruction's negate-A bit), issued by one thread, asynchronously: they run while the CTA
+// gathers and row-transforms the NEXT batch.  gather / rows / unpack are the fused kernel's.
+//   convert   row-pass output (fp32, gh) -> four BF16 operands Hr_hi, Hr_lo, Hi_hi, Hi_lo in the
+//             K-major core-matrix layout (epic_packed.cuh), 16-byte stores
+//   issue     one thread: 24 x tcgen05.mma + tcgen05.commit -> mbarrier
+//   epilogue  (one batch later) thread = (image row m = TMEM lane, 16 columns l1): tcgen05.ld of
+//             D_r / D_i, S5 products, S6 accumulation in registers
+// One CTA per SM (185 KB of shared memory, all 512 TMEM columns).
+constexpr int TC_N = 128, TC_NT = 256, TC_NG = F * 2 * S;  // image side, threads, GEMM N = (pair, pol, l1)
+constexpr int TC_A_MAT = 4 * TC_N * 8;                       // bf16 elements of one A matrix: [4 K chunks][128 m][8]
+constexpr int TC_B_MAT = 4 * TC_NG * 8;                      // of one B matrix: [4 K chunks][256 n][8]
+
+__device__ __forceinline__ void bf16_split2(float a, float b, uint32_t& hi, uint32_t& lo) {
+  __nv_bfloat162 h = __floats2bfloat162_rn(a, b);  // .x = a = lower address
+  hi = *reinterpret_cast<uint32_t*>(&h);
+  __nv_bfloat162 l = __floats2bfloat162_rn(a - __uint_as_float(hi << 16), b - __uint_as_float(hi & 0xFFFF0000u));
+  lo = *reinterpret_cast<uint32_t*>(&l);
+}
+
+// gh[f][y][l1] = (re_X, re_Y, im_X, im_Y) -> B matrices 0 Hr_hi, 1 Hr_lo, 2 Hi_hi, 3 Hi_lo at
+// [K chunk y / 8][n = f * 64 + pol * 32 + l1][y % 8]
+__device__ __forceinline__ void tc_convert(const float4* __restrict__ gh, uint16_t* __restrict__ sB, int tid) {
+  for (int item = tid; item < F * S * 4; item += TC_NT) {
+    const int l1 = item & 31, j = (item >> 5) & 3, f = item >> 7;
+    float v[4][8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const float4 c = gh[f * PLANE + (8 * j + i) * HS + l1];
+      v[0][i] = c.x; v[1][i] = c.y; v[2][i] = c.z; v[3][i] = c.w;
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const int pol = q & 1, ri = q >> 1;
+      uint32_t hi[4], lo[4];
+#pragma unroll
+      for (int e = 0; e < 4; ++e) bf16_split2(v[q][2 * e], v[q][2 * e + 1], hi[e], lo[e]);
+      const int n = f * 64 + pol * 32 + l1;
+      uint16_t* d = sB + (size_t)(2 * ri) * TC_B_MAT + (size_t)(j * TC_NG + n) * 8;
+      *reinterpret_cast<uint4*>(d) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+      *reinterpret_cast<uint4*>(d + TC_B_MAT) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+    }
+  }
+}
+
+// A matrices 0 Fr_hi, 1 Fr_lo, 2 Fi_hi, 3 Fi_lo; D_r at TMEM columns [0, 256), D_i at [256, 512)
+__device__ __forceinline__ void tc_issue(uint32_t sA, uint32_t sB, uint32_t tbase, uint64_t* bar) {
+  constexpr uint32_t A_LBO = TC_N * 16, B_LBO = TC_NG * 16, SBO = 128;
+  constexpr uint32_t A_BYTES = TC_A_MAT * 2, B_BYTES = TC_B_MAT * 2;
+  constexpr uint32_t ID = umma_idesc_bf16(128, TC_NG, false), IDN = umma_idesc_bf16(128, TC_NG, true);
+  uint32_t acc = 0u;
+  auto term = [&](uint32_t d, uint32_t am, uint32_t bm, uint32_t idesc) {
+#pragma unroll
+    for (uint32_t s = 0; s < 2; ++s) {  // K = 32 = two K = 16 steps
+      umma_bf16(d, umma_desc(sA + am * A_BYTES + s * 2 * A_LBO, A_LBO, SBO),
+                umma_desc(sB + bm * B_BYTES + s * 2 * B_LBO, B_LBO, SBO), idesc, acc);
+      acc = 1u;
+    }
+  };
+  const uint32_t dr = tbase, di = tbase + 256;
+  term(dr, 0, 0, ID); term(dr, 0, 1, ID); term(dr, 1, 0, ID);      //  Fr Hr
+  term(dr, 2, 2, IDN); term(dr, 2, 3, IDN); term(dr, 3, 2, IDN);   // -Fi Hi
+  acc = 0u;
+  term(di, 2, 0, ID); term(di, 2, 1, ID); term(di, 3, 0, ID);      //  Fi Hr
+  term(di, 0, 2, ID); term(di, 0, 3, ID); term(di, 1, 2, ID);      //  Fr Hi
+  umma_commit(bar);
+}
+
+// S5 + S6 from the accumulators in tensor memory: acc[q * 16 + k], q = XX, YY, Re XY, Im XY, k = l1 - 16 hh
+template <int NPROD>
+__device__ __forceinline__ void tc_epilogue(uint32_t tlane, float (&acc)[NPROD == 4 ? 64 : 32]) {
+#pragma unroll 1
+  for (int f = 0; f < F; ++f) {
+    uint32_t rx[16], ry[16], ix[16], iy[16];
+    tmem_ld16_issue(tlane + f * 64, rx);
+    tmem_ld16_issue(tlane + f * 64 + 32, ry);
+    tmem_ld16_issue(tlane + 256 + f * 64, ix);
+    tmem_ld16_issue(tlane + 256 + f * 64 + 32, iy);
+    tmem_wait_ld();
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+      const float a = __uint_as_float(rx[k]), b = __uint_as_float(ix[k]);
+      const float c = __uint_as_float(ry[k]), d = __uint_as_float(iy[k]);
+      acc[k] = fmaf(a, a, fmaf(b, b, acc[k]));
+      acc[16 + k] = fmaf(c, c, fmaf(d, d, acc[16 + k]));
+      if constexpr (NPROD == 4) {  // XY = A_X conj(A_Y) (reading Q11)
+        acc[32 + k] = fmaf(a, c, fmaf(b, d, acc[32 + k]));
+        acc[48 + k] = fmaf(b, c, fmaf(-a, d, acc[48 + k]));
+      }
+    }
+  }
+}
+
+template <int NPROD, bool DELTA, int NB>
+__global__ void __launch_bounds__(TC_NT, 1) epic_tc_kernel(FusedParams P, const uint4* __restrict__ a_tab) {
+  constexpr int Q = 4, NT = TC_NT, N = TC_N, NACC = NPROD == 4 ? 4 : 2;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  float4* gh = reinterpret_cast<float4*>(smem_raw);  // [F][32][HS]
+  float4* tws = gh + F * PLANE;                      // [2Q][TWV]
+  float4* E = tws + 2 * Q * TWV;                     // [F][A]
+  uint16_t* sA = reinterpret_cast<uint16_t*>(
+      smem_raw + (((size_t)(F * PLANE + 2 * Q * TWV + F * P.n_ant) * sizeof(float4) + 127) & ~(size_t)127));
+  uint16_t* sB = sA + 4 * TC_A_MAT;
+  __shared__ uint32_t tmem_slot;
+  __shared__ __align__(8) uint64_t bar;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+  const long long g0 = P.total * (long long)blockIdx.x / gridDim.x;
+  const long long g1 = P.total * (long long)(blockIdx.x + 1) / gridDim.x;
+  if (g0 >= g1) return;
+  int unit = (int)(g0 / P.nb);
+  uint2 info[S * S / NT];
+#pragma unroll
+  for (int j = 0; j < S * S / NT; ++j) info[j] = __ldg(P.cell_info + tid + j * NT);
+  for (int i = tid; i < F * PLANE; i += NT) gh[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);  // rows >= R stay zero
+  for (int i = tid; i < 2 * Q * TWV; i += NT) tws[i] = __ldg(P.tw + i);
+  for (int i = tid; i < 4 * TC_A_MAT / 8; i += NT) reinterpret_cast<uint4*>(sA)[i] = __ldg(a_tab + i);
+  if (tid == 0) mbar_init(&bar, 1u);
+  fence_smem_to_async_proxy();  // the A operand is read by the tensor cores (async proxy)
+  const uint32_t tbase = tmem_alloc_cta<512>(&tmem_slot, warp);  // includes the CTA barrier
+  // epilogue role: image row m = TMEM lane (a warp reaches the 32 lanes of quadrant warp % 4), columns l1 = 16 hh + k
+  const int m_row = (warp & 3) * 32 + lane, hh = warp >> 2;
+  const uint32_t tlane = tbase + ((uint32_t)((warp & 3) * 32) << 16) + 16u * (uint32_t)hh;
+  const uint32_t sA_u = (uint32_t)__cvta_generic_to_shared(sA), sB_u = (uint32_t)__cvta_generic_to_shared(sB);
+
+  float acc[NPROD == 4 ? 64 : 32];
+#pragma unroll
+  for (int k = 0; k < (NPROD == 4 ? 64 : 32); ++k) acc[k] = 0.0f;
+
+  auto flush = [&](int u, bool complete, int slot) {  // as in epic_fused_kernel, other thread <-> pixel mapping
+    const int c = u / Q, l2 = u - c * Q;
+    const size_t plane = (size_t)N * N;
+    float* o = P.out + (size_t)c * P.n_planes * plane + (size_t)m_row * N + Q * 16 * hh + l2;
+    float* part = P.partial + ((size_t)(blockIdx.x * 2 + slot) * NACC * 16) * NT + tid;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+      float v[NACC];
+#pragma unroll
+      for (int q = 0; q < NACC; ++q) { v[q] = acc[q * 16 + k]; acc[q * 16 + k] = 0.0f; }
+      if (complete) {
+        add_pixel<NPROD>(o + Q * k, plane, v);
+      } else {
+#pragma unroll
+        for (int q = 0; q < NACC; ++q) part[(size_t)(q * 16 + k) * NT] = v[q];
+      }
+    }
+  };
+
+  int b = (int)(g0 - (long long)unit * P.nb);
+  const int first_unit = unit;
+  int seg_begin = b;
+  PrefetchSlots ps;
+  prefetch_init<NT>(P, tid, ps);
+  uint32_t wlo[MAXW], whi[MAXW];
+  prefetch_batch<NT>(P, ps, unit / Q, b, wlo, whi);
+  unpack_batch(P, ps, E, wlo, whi, unit / Q);
+  __syncthreads();
+
+  // the batch whose MMAs are in flight: its epilogue (and its unit's flush) happen one iteration later
+  bool pend = false, pend_flush = false, pend_complete = false;
+  int pend_unit = 0, pend_slot = 0;
+  uint32_t phase = 0u;
+  auto retire = [&]() {
+    mbar_wait(&bar, phase);
+    phase ^= 1u;
+    tc_fence_after_sync();
+    tc_epilogue<NPROD>(tlane, acc);
+    if (pend_flush) flush(pend_unit, pend_complete, pend_slot);
+    pend = false;
+  };
+
+  const int ntask = F * P.R * 2;
+  for (long long g = g0; g < g1; ++g) {
+    int unit_n = unit, b_n = b + 1;
+    if (b_n == P.nb) { b_n = 0; ++unit_n; }
+    const bool more = g + 1 < g1;
+    if (more) prefetch_batch<NT>(P, ps, unit_n / Q, b_n, wlo, whi);
+
+    gather_batch<NT, DELTA>(P, E, gh, info);
+    __syncthreads();
+
+    const int l2 = unit % Q;
+    for (int base = warp * 32; base < ntask; base += NT) {
+      const int task = base + lane;
+      const bool valid = task < ntask;
+      int f = 0, y = S - 1, h = 0;
+      if (valid) { h = task & 1; const int p = task >> 1; f = p / P.R; y = p - f * P.R; }
+      row_task<NB>(gh + f * PLANE + y * HS, tws + (l2 + Q * h) * TWV, h, valid);
+    }
+    __syncthreads();
+
+    if (more) unpack_batch(P, ps, E, wlo, whi, unit_n / Q);  // E was last read by this batch's gather
+    if (pend) retire();            // the previous batch: D -> products -> registers; frees D and the B operands
+    tc_convert(gh, sB, tid);
+    fence_smem_to_async_proxy();
+    tc_fence_before_sync();
+    __syncthreads();               // B complete, every thread done reading D; gh is free for the next gather
+    if (tid == 0) {
+      tc_fence_after_sync();
+      tc_issue(sA_u, sB_u, tbase, &bar);
+    }
+    pend = true;
+    pend_unit = unit;
+    pend_flush = unit_n != unit || !more;
+    pend_complete = seg_begin == 0 && b == P.nb - 1;
+    pend_slot = unit == first_unit ? 0 : 1;
+    if (pend_flush) seg_begin = 0;
+    unit = unit_n; b = b_n;
+  }
+  if (pend) retire();
+  tmem_free_cta<512>(tbase, warp);
+}
+
 struct FusedTables {
   uint2* cell_info;
   float4* tw;
+  uint4* a_tab;  // tensor-core path: the DFT matrix as BF16 hi/lo operands (Q = 4 only), or nullptr
 };
 
 template <int Q>
@@ -565,12 +799,46 @@ int fused_plan_init(epic_plan* p) {
     for (int j = 0; j < TWV; ++j)
       tw[(size_t)rho * TWV + j] = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
   }
+  // tensor-core path (Q = 4): F[m][y] = exp(+2 pi i m y / N), m < 128, y < 32, from double, split
+  // hi + lo in BF16; matrices Fr_hi, Fr_lo, Fi_hi, Fi_lo, each [K chunk y / 8][m][y % 8]
+  std::vector<uint16_t> a_tab;
+  if (Q == 4) {
+    auto bf16_rn = [](float v) {
+      uint32_t u;
+      std::memcpy(&u, &v, 4);
+      return (uint16_t)((u + 0x7FFFu + ((u >> 16) & 1u)) >> 16);
+    };
+    auto bf16_f = [](uint16_t h) {
+      const uint32_t u = (uint32_t)h << 16;
+      float f;
+      std::memcpy(&f, &u, 4);
+      return f;
+    };
+    a_tab.assign((size_t)4 * TC_A_MAT, 0);
+    for (int m = 0; m < TC_N; ++m)
+      for (int y = 0; y < S; ++y) {
+        const double ang = 2.0 * M_PI * (double)((m * y) % p->N) / (double)p->N;
+        const double v[2] = {std::cos(ang), std::sin(ang)};
+        for (int ri = 0; ri < 2; ++ri) {
+          const uint16_t hi = bf16_rn((float)v[ri]);
+          const uint16_t lo = bf16_rn((float)(v[ri] - (double)bf16_f(hi)));
+          const size_t at = ((size_t)(y >> 3) * TC_N + m) * 8 + (y & 7);
+          a_tab[(size_t)(2 * ri) * TC_A_MAT + at] = hi;
+          a_tab[(size_t)(2 * ri + 1) * TC_A_MAT + at] = lo;
+        }
+      }
+  }
   FusedTables* ft = new (std::nothrow) FusedTables();
   if (!ft) return EPIC_ERR_NOMEM;
   ft->cell_info = nullptr;
   ft->tw = nullptr;
+  ft->a_tab = nullptr;
   cudaError_t ce = cudaMalloc(&ft->cell_info, info.size() * sizeof(uint2));
   if (ce == cudaSuccess) ce = cudaMalloc(&ft->tw, tw.size() * sizeof(float4));
+  if (ce == cudaSuccess && !a_tab.empty()) {
+    ce = cudaMalloc(&ft->a_tab, a_tab.size() * sizeof(uint16_t));
+    if (ce == cudaSuccess) ce = cudaMemcpy(ft->a_tab, a_tab.data(), a_tab.size() * sizeof(uint16_t), cudaMemcpyHostToDevice);
+  }
   if (ce == cudaSuccess)
     ce = cudaMemcpy(ft->cell_info, info.data(), info.size() * sizeof(uint2), cudaMemcpyHostToDevice);
   if (ce == cudaSuccess) ce = cudaMemcpy(ft->tw, tw.data(), tw.size() * sizeof(float4), cudaMemcpyHostToDevice);
@@ -578,6 +846,7 @@ int fused_plan_init(epic_plan* p) {
     set_cuda_error(ce);
     if (ft->cell_info) cudaFree(ft->cell_info);
     if (ft->tw) cudaFree(ft->tw);
+    if (ft->a_tab) cudaFree(ft->a_tab);
     delete ft;
     return ce == cudaErrorMemoryAllocation ? EPIC_ERR_NOMEM : EPIC_ERR_CUDA;
   }
@@ -591,6 +860,7 @@ void fused_plan_free(epic_plan* p) {
   if (ft) {
     if (ft->cell_info) cudaFree(ft->cell_info);
     if (ft->tw) cudaFree(ft->tw);
+    if (ft->a_tab) cudaFree(ft->a_tab);
     delete ft;
   }
   p->d_fused = nullptr;
@@ -608,10 +878,35 @@ int fused_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products) 
   return smem <= (size_t)200 * 1024 ? 1 : 0;
 }
 
-int fused_image(epic_plan* p, const ImageArgs& a) {
+static size_t tc_smem_bytes(int n_ant) {
+  const size_t head = ((size_t)F * PLANE + (size_t)2 * 4 * TWV + (size_t)F * n_ant) * sizeof(float4);
+  return ((head + 127) & ~(size_t)127) + (size_t)4 * (TC_A_MAT + TC_B_MAT) * sizeof(uint16_t);
+}
+
+int tensor_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products) {
+  if (!fused_supported(p, is_cf32, n_pol, n_products)) return 0;
+  const FusedTables* ft = static_cast<const FusedTables*>(p->d_fused);
+  if (p->N != TC_N || !ft->a_tab || n_pol != 2 || p->n_layout != 1) return 0;
+  return tc_smem_bytes(p->n_ant) <= (size_t)226 * 1024 ? 1 : 0;
+}
+
+template <int NPROD, bool DELTA, int NB>
+static int launch_tc(const epic_plan* p, const FusedParams& P, const uint4* a_tab, cudaStream_t s) {
+  const size_t smem = tc_smem_bytes(P.n_ant);
+  auto kern = epic_tc_kernel<NPROD, DELTA, NB>;
+  EPIC_CUDA_TRY(cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int grid = (int)std::min<long long>(P.total, p->n_sm);  // one CTA per SM (shared memory, all of TMEM)
+  constexpr int NACC = NPROD == 4 ? 4 : 2;
+  if ((size_t)grid * 2 * NACC * 16 * TC_NT * sizeof(float) > p->scratch_bytes) return EPIC_ERR_RANGE;
+  kern<<<grid, TC_NT, smem, s>>>(P, a_tab);
+  epic_fused_fixup<4, NPROD, true><<<(unsigned)(P.total / P.nb), TC_NT, 0, s>>>(P, grid);
+  EPIC_CUDA_TRY(cudaGetLastError());
+  return EPIC_OK;
+}
+
+static void fill_params(const epic_plan* p, const ImageArgs& a, FusedParams& P) {
   const FusedTables* ft = static_cast<const FusedTables*>(p->d_fused);
   const int Q = p->N / S;
-  FusedParams P;
   P.volt = static_cast<const uint8_t*>(a.volt);
   P.out = a.out;
   P.cell_info = ft->cell_info;
@@ -632,6 +927,32 @@ int fused_image(epic_plan* p, const ImageArgs& a) {
   const int per_batch = a.n_pol == 2 ? F : 2 * F;  // time samples per batch
   P.nb = (a.n_t + per_batch - 1) / per_batch;
   P.total = (long long)a.n_chan * Q * P.nb;
+}
+
+int tensor_image(epic_plan* p, const ImageArgs& a) {
+  const FusedTables* ft = static_cast<const FusedTables*>(p->d_fused);
+  FusedParams P;
+  fill_params(p, a, P);
+  const bool delta = p->t.is_delta != 0, nb12 = std::max(p->R, p->Cc) <= 16 + 12;
+  int st;
+#define EPIC_TC_CASE(NPROD, DELTA, NB) st = launch_tc<NPROD, DELTA, NB>(p, P, ft->a_tab, a.stream)
+  if (a.n_products == 2) {
+    if (delta) { if (nb12) EPIC_TC_CASE(2, true, 12); else EPIC_TC_CASE(2, true, 16); }
+    else { if (nb12) EPIC_TC_CASE(2, false, 12); else EPIC_TC_CASE(2, false, 16); }
+  } else {
+    if (delta) { if (nb12) EPIC_TC_CASE(4, true, 12); else EPIC_TC_CASE(4, true, 16); }
+    else { if (nb12) EPIC_TC_CASE(4, false, 12); else EPIC_TC_CASE(4, false, 16); }
+  }
+#undef EPIC_TC_CASE
+  if (st != EPIC_OK) return st;
+  p->last_launches = 2;
+  return EPIC_OK;
+}
+
+int fused_image(epic_plan* p, const ImageArgs& a) {
+  const int Q = p->N / S;
+  FusedParams P;
+  fill_params(p, a, P);
   int st;
   if (Q == 2) st = launch_fused_q<2>(p, P, a.n_products, a.stream);
   else st = launch_fused_q<4>(p, P, a.n_products, a.stream);

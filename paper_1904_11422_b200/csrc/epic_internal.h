@@ -87,6 +87,8 @@ int fused_plan_init(epic_plan* p);  // sets p->fused_ok, allocates p->d_fused
 void fused_plan_free(epic_plan* p);
 int fused_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products);
 int fused_image(epic_plan* p, const ImageArgs& a);
+int tensor_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products);  // tensor-core column pass
+int tensor_image(epic_plan* p, const ImageArgs& a);
 
 // epic_tiled.cu
 int tiled_plan_init(epic_plan* p);  // sets p->tiled_ok, allocates p->d_tiled

@@ -221,6 +221,10 @@ static int image_common(epic_plan* plan, const void* volt, int is_cf32, int n_t,
     if (!tiled_can) return EPIC_ERR_RANGE;
     return tiled_image(plan, a);
   }
+  if (path == EPIC_PATH_TENSOR) {
+    if (!fused_can || !tensor_supported(plan, is_cf32, n_pol, n_products)) return EPIC_ERR_RANGE;
+    return tensor_image(plan, a);
+  }
   return twopass_image(plan, a);
 }
 
@@ -390,8 +394,10 @@ int epic_plan_set_scratch_limit(epic_plan* plan, long long bytes) {
 
 int epic_plan_set_path(epic_plan* plan, int path) {
   if (!plan) return EPIC_ERR_ARG;
-  if (path != EPIC_PATH_AUTO && path != EPIC_PATH_TWOPASS && path != EPIC_PATH_FUSED && path != EPIC_PATH_TILED)
+  if (path != EPIC_PATH_AUTO && path != EPIC_PATH_TWOPASS && path != EPIC_PATH_FUSED && path != EPIC_PATH_TILED &&
+      path != EPIC_PATH_TENSOR)
     return EPIC_ERR_ARG;
+  if (path == EPIC_PATH_TENSOR && (!plan->fused_ok || plan->N != 128 || plan->n_layout != 1)) return EPIC_ERR_RANGE;
   if (path == EPIC_PATH_FUSED && !plan->fused_ok) return EPIC_ERR_RANGE;
   if (path == EPIC_PATH_TILED && !plan->tiled_ok) return EPIC_ERR_RANGE;
   plan->path_req = path;

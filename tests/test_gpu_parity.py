@@ -7,7 +7,7 @@ import pytest
 from oracle import epic_oracle as orc
 from workloads import make_config, make_custom, make_per_channel
 
-from epic_testlib import TOL, assert_parity, run_gpu, run_oracle
+from epic_testlib import TOL, assert_parity, max_rel_err, run_gpu, run_oracle
 
 pytestmark = pytest.mark.gpu
 
@@ -517,3 +517,39 @@ def test_per_channel_full_size_lwa_band():
     assert np.isfinite(gpu).all() and (gpu >= 0).all()
     totals = gpu[:, 0].sum(axis=(1, 2))
     assert totals.min() > 0.5 * totals.max()
+
+
+# ------------------------------------------------------------------ tensor-core column pass
+TENSOR_CASES = [
+    make_config(2, n_chan=3, n_t=37),                       # delta kernel, XX/YY, ragged last batch
+    make_config(3, n_chan=2, n_t=29),                       # 3x3 taps, four products, point source
+    make_config(2, n_chan=1, n_t=1),                        # one frame: no averaging of the BF16 split error
+    make_config(3, n_chan=5, n_t=300),                      # units split between CTAs (fix-up kernel)
+    make_custom(grid_n=64, pad=2, n_ant=64, n_pol=2, kernel_k=5, n_chan=2, n_t=9, layout="disc", n_sources=2),
+]
+
+
+@pytest.mark.parametrize("wl", TENSOR_CASES, ids=lambda w: f"{w.name}-c{w.n_chan}-t{w.n_t}")
+def test_tensor_core_path_matches_oracle(wl):
+    """EPIC_PATH_TENSOR: the column transform as a BF16 hi/lo-split contraction on tcgen05 tensor
+    cores, same 1e-4-of-peak bar as the FP32 paths, and the same answer as the fused kernel."""
+    v = wl.voltages()
+    gpu, info = run_gpu(wl, volt=v, path=4, calls=2, return_plan_info=True)
+    assert info["path"] == 4 and info["launches"] == 2
+    ref = run_oracle(wl, volt=v)
+    assert_parity(gpu, ref, what=f"{wl.name} tensor path")
+    fused = run_gpu(wl, volt=v, path=2, calls=2)
+    assert max_rel_err(gpu, fused.astype(np.float64)) <= TOL
+
+
+def test_tensor_core_path_is_bit_reproducible_and_rejected_where_unsupported():
+    epic = _epic()
+    wl = TENSOR_CASES[3]
+    v = wl.voltages()
+    a = run_gpu(wl, volt=v, path=4)
+    b = run_gpu(wl, volt=v, path=4)
+    assert np.array_equal(a, b)
+    small = make_config(1)
+    with epic.Plan(small.grid_n, small.pad, small.ant_uv, small.taps, small.kernel_k) as plan:
+        with pytest.raises(epic.EpicError):
+            plan.set_path(epic.EPIC_PATH_TENSOR)
