@@ -40,6 +40,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <type_traits>
 #include <vector>
 
 #include <cuda_bf16.h>
@@ -249,7 +250,8 @@ __device__ __forceinline__ void add_pixel(float* __restrict__ px, size_t plane, 
 // order.  One CTA per unit, same thread <-> pixel mapping as the main kernel.
 template <int Q, int NPROD, bool TC = false>
 __global__ void __launch_bounds__(64 * Q) epic_fused_fixup(FusedParams P, int main_grid) {
-  constexpr int NT = 64 * Q, N = 32 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
+  // NT threads with KPT pixels each, as in the main kernel (the tensor-core kernel: its 256 epilogue threads)
+  constexpr int NT = 64 * Q, KPT = 16, N = 32 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
   const int unit = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const long long G = main_grid, first = (long long)unit * P.nb, last = first + P.nb - 1;
   const int b_lo = (int)(((first + 1) * G - 1) / P.total), b_hi = (int)(((last + 1) * G - 1) / P.total);
@@ -261,18 +263,18 @@ __global__ void __launch_bounds__(64 * Q) epic_fused_fixup(FusedParams P, int ma
   float* o = P.out + (size_t)c * P.n_planes * plane + (Q * l1 + l2) + (size_t)rho * N;
   size_t kstride = (size_t)2 * Q * N;
   if constexpr (TC) {  // tensor-core kernel: thread = (image row m, 16 columns l1), see epic_tc_kernel
-    o = P.out + (size_t)c * P.n_planes * plane + (size_t)((warp & 3) * 32 + lane) * N + Q * 16 * (warp >> 2) + l2;
+    o = P.out + (size_t)c * P.n_planes * plane + (size_t)((warp & 3) * 32 + lane) * N + Q * KPT * (warp >> 2) + l2;
     kstride = Q;
   }
-  for (int k = 0; k < 16; ++k) {
+  for (int k = 0; k < KPT; ++k) {
     float v[NACC];
 #pragma unroll
     for (int q = 0; q < NACC; ++q) v[q] = 0.0f;
     for (int b = b_lo; b <= b_hi; ++b) {
       const int slot = (first <= P.total * b / G) ? 0 : 1;  // does the segment start the CTA's range?
-      const float* part = P.partial + ((size_t)(b * 2 + slot) * NACC * 16) * NT + tid;
+      const float* part = P.partial + ((size_t)(b * 2 + slot) * NACC * KPT) * NT + tid;
 #pragma unroll
-      for (int q = 0; q < NACC; ++q) v[q] += part[(size_t)(q * 16 + k) * NT];
+      for (int q = 0; q < NACC; ++q) v[q] += part[(size_t)(q * KPT + k) * NT];
     }
     add_pixel<NPROD>(o + k * kstride, plane, v);
   }
@@ -489,7 +491,9 @@ epic_fused_kernel(FusedParams P) {
 //   epilogue  (one batch later) thread = (image row m = TMEM lane, 16 columns l1): tcgen05.ld of
 //             D_r / D_i, S5 products, S6 accumulation in registers
 // One CTA per SM (185 KB of shared memory, all 512 TMEM columns).
-constexpr int TC_N = 128, TC_NT = 256, TC_NG = F * 2 * S;  // image side, threads, GEMM N = (pair, pol, l1)
+constexpr int TC_N = 128, TC_NT = 512, TC_NG = F * 2 * S;  // image side, threads, GEMM N = (pair, pol, l1)
+constexpr int TC_EPI_NT = 256;                               // threads of the epilogue role (warps 8-15)
+constexpr int TC_KPT = TC_N * S / TC_EPI_NT;                 // image pixels per epilogue thread (16 columns l1 of one row m)
 constexpr int TC_A_MAT = 4 * TC_N * 8;                       // bf16 elements of one A matrix: [4 K chunks][128 m][8]
 constexpr int TC_B_MAT = 4 * TC_NG * 8;                      // of one B matrix: [4 K chunks][256 n][8]
 
@@ -548,31 +552,50 @@ __device__ __forceinline__ void tc_issue(uint32_t sA, uint32_t sB, uint32_t tbas
   umma_commit(bar);
 }
 
-// S5 + S6 from the accumulators in tensor memory: acc[q * 16 + k], q = XX, YY, Re XY, Im XY, k = l1 - 16 hh
-template <int NPROD>
-__device__ __forceinline__ void tc_epilogue(uint32_t tlane, float (&acc)[NPROD == 4 ? 64 : 32]) {
-#pragma unroll 1
-  for (int f = 0; f < F; ++f) {
-    uint32_t rx[16], ry[16], ix[16], iy[16];
-    tmem_ld16_issue(tlane + f * 64, rx);
-    tmem_ld16_issue(tlane + f * 64 + 32, ry);
-    tmem_ld16_issue(tlane + 256 + f * 64, ix);
-    tmem_ld16_issue(tlane + 256 + f * 64 + 32, iy);
-    tmem_wait_ld();
+template <int NPROD, int K0>
+__device__ __forceinline__ void tc_products(const uint32_t (&rx)[8], const uint32_t (&ry)[8], const uint32_t (&ix)[8],
+                                            const uint32_t (&iy)[8], float (&acc)[(NPROD == 4 ? 4 : 2) * TC_KPT]) {
 #pragma unroll
-    for (int k = 0; k < 16; ++k) {
-      const float a = __uint_as_float(rx[k]), b = __uint_as_float(ix[k]);
-      const float c = __uint_as_float(ry[k]), d = __uint_as_float(iy[k]);
-      acc[k] = fmaf(a, a, fmaf(b, b, acc[k]));
-      acc[16 + k] = fmaf(c, c, fmaf(d, d, acc[16 + k]));
-      if constexpr (NPROD == 4) {  // XY = A_X conj(A_Y) (reading Q11)
-        acc[32 + k] = fmaf(a, c, fmaf(b, d, acc[32 + k]));
-        acc[48 + k] = fmaf(b, c, fmaf(-a, d, acc[48 + k]));
-      }
+  for (int k = 0; k < 8; ++k) {
+    const float a = __uint_as_float(rx[k]), b = __uint_as_float(ix[k]);
+    const float c = __uint_as_float(ry[k]), d = __uint_as_float(iy[k]);
+    acc[K0 + k] = fmaf(a, a, fmaf(b, b, acc[K0 + k]));
+    acc[TC_KPT + K0 + k] = fmaf(c, c, fmaf(d, d, acc[TC_KPT + K0 + k]));
+    if constexpr (NPROD == 4) {  // XY = A_X conj(A_Y) (reading Q11)
+      acc[2 * TC_KPT + K0 + k] = fmaf(a, c, fmaf(b, d, acc[2 * TC_KPT + K0 + k]));
+      acc[3 * TC_KPT + K0 + k] = fmaf(b, c, fmaf(-a, d, acc[3 * TC_KPT + K0 + k]));
     }
   }
 }
 
+// S5 + S6 from the accumulators in tensor memory: acc[q * KPT + k], q = XX, YY, Re XY, Im XY, k = l1 - KPT cg
+template <int NPROD>
+__device__ __forceinline__ void tc_epilogue(uint32_t tlane, float (&acc)[(NPROD == 4 ? 4 : 2) * TC_KPT]) {
+  static_assert(TC_KPT == 16, "two tcgen05.ld .x8 per quantity below");
+  // 8 columns at a time: 32 registers of loads in flight beside the (up to 64) accumulators
+#pragma unroll 1
+  for (int fh = 0; fh < 2 * F; ++fh) {
+    const int f = fh >> 1, k0 = (fh & 1) * 8;
+    uint32_t rx[8], ry[8], ix[8], iy[8];
+    tmem_ld8_issue(tlane + f * 64 + k0, rx);
+    tmem_ld8_issue(tlane + f * 64 + 32 + k0, ry);
+    tmem_ld8_issue(tlane + 256 + f * 64 + k0, ix);
+    tmem_ld8_issue(tlane + 256 + f * 64 + 32 + k0, iy);
+    tmem_wait_ld();
+    if (fh & 1) {
+      tc_products<NPROD, 8>(rx, ry, ix, iy, acc);
+    } else {
+      tc_products<NPROD, 0>(rx, ry, ix, iy, acc);
+    }
+  }
+}
+
+__device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0;\n" ::: "memory"); }
+
+// 512 threads in two roles that share gather / unpack / convert and split the middle of a batch:
+// warps 0-7 run the row transforms of batch i while warps 8-15 take batch i-1's accumulators out
+// of tensor memory (products, sums, flush).  The roles are two instantiations of one loop, so the
+// image accumulators are registers of the epilogue warps only.
 template <int NPROD, bool DELTA, int NB>
 __global__ void __launch_bounds__(TC_NT, 1) epic_tc_kernel(FusedParams P, const uint4* __restrict__ a_tab) {
   constexpr int Q = 4, NT = TC_NT, N = TC_N, NACC = NPROD == 4 ? 4 : 2;
@@ -590,106 +613,120 @@ __global__ void __launch_bounds__(TC_NT, 1) epic_tc_kernel(FusedParams P, const 
   const long long g0 = P.total * (long long)blockIdx.x / gridDim.x;
   const long long g1 = P.total * (long long)(blockIdx.x + 1) / gridDim.x;
   if (g0 >= g1) return;
-  int unit = (int)(g0 / P.nb);
-  uint2 info[S * S / NT];
-#pragma unroll
-  for (int j = 0; j < S * S / NT; ++j) info[j] = __ldg(P.cell_info + tid + j * NT);
   for (int i = tid; i < F * PLANE; i += NT) gh[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);  // rows >= R stay zero
   for (int i = tid; i < 2 * Q * TWV; i += NT) tws[i] = __ldg(P.tw + i);
   for (int i = tid; i < 4 * TC_A_MAT / 8; i += NT) reinterpret_cast<uint4*>(sA)[i] = __ldg(a_tab + i);
   if (tid == 0) mbar_init(&bar, 1u);
   fence_smem_to_async_proxy();  // the A operand is read by the tensor cores (async proxy)
   const uint32_t tbase = tmem_alloc_cta<512>(&tmem_slot, warp);  // includes the CTA barrier
-  // epilogue role: image row m = TMEM lane (a warp reaches the 32 lanes of quadrant warp % 4), columns l1 = 16 hh + k
-  const int m_row = (warp & 3) * 32 + lane, hh = warp >> 2;
-  const uint32_t tlane = tbase + ((uint32_t)((warp & 3) * 32) << 16) + 16u * (uint32_t)hh;
   const uint32_t sA_u = (uint32_t)__cvta_generic_to_shared(sA), sB_u = (uint32_t)__cvta_generic_to_shared(sB);
 
-  float acc[NPROD == 4 ? 64 : 32];
+  auto run = [&](auto role) {
+    constexpr bool EPI = decltype(role)::value;
+    // epilogue role: image row m = TMEM lane (a warp reaches the 32 lanes of quadrant warp % 4),
+    // columns l1 = KPT cg + k; etid = thread index among the 256 epilogue threads
+    const int etid = tid - TC_EPI_NT, m_row = (warp & 3) * 32 + lane, cg = (warp >> 2) & 1;
+    const uint32_t tlane = tbase + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(TC_KPT * cg);
+    float acc[EPI ? NACC * TC_KPT : 1];
 #pragma unroll
-  for (int k = 0; k < (NPROD == 4 ? 64 : 32); ++k) acc[k] = 0.0f;
+    for (int k = 0; k < (EPI ? NACC * TC_KPT : 1); ++k) acc[k] = 0.0f;
 
-  auto flush = [&](int u, bool complete, int slot) {  // as in epic_fused_kernel, other thread <-> pixel mapping
-    const int c = u / Q, l2 = u - c * Q;
-    const size_t plane = (size_t)N * N;
-    float* o = P.out + (size_t)c * P.n_planes * plane + (size_t)m_row * N + Q * 16 * hh + l2;
-    float* part = P.partial + ((size_t)(blockIdx.x * 2 + slot) * NACC * 16) * NT + tid;
+    auto flush = [&](int u, bool complete, int slot) {  // as in epic_fused_kernel, other thread <-> pixel mapping
+      if constexpr (EPI) {
+        const int c = u / Q, l2 = u - c * Q;
+        const size_t plane = (size_t)N * N;
+        float* o = P.out + (size_t)c * P.n_planes * plane + (size_t)m_row * N + Q * TC_KPT * cg + l2;
+        float* part = P.partial + ((size_t)(blockIdx.x * 2 + slot) * NACC * TC_KPT) * TC_EPI_NT + etid;
 #pragma unroll
-    for (int k = 0; k < 16; ++k) {
-      float v[NACC];
+        for (int k = 0; k < TC_KPT; ++k) {
+          float v[NACC];
 #pragma unroll
-      for (int q = 0; q < NACC; ++q) { v[q] = acc[q * 16 + k]; acc[q * 16 + k] = 0.0f; }
-      if (complete) {
-        add_pixel<NPROD>(o + Q * k, plane, v);
-      } else {
+          for (int q = 0; q < NACC; ++q) { v[q] = acc[q * TC_KPT + k]; acc[q * TC_KPT + k] = 0.0f; }
+          if (complete) {
+            add_pixel<NPROD>(o + Q * k, plane, v);
+          } else {
 #pragma unroll
-        for (int q = 0; q < NACC; ++q) part[(size_t)(q * 16 + k) * NT] = v[q];
+            for (int q = 0; q < NACC; ++q) part[(size_t)(q * TC_KPT + k) * TC_EPI_NT] = v[q];
+          }
+        }
       }
+    };
+
+    int unit = (int)(g0 / P.nb);
+    uint2 info[S * S / NT];
+#pragma unroll
+    for (int j = 0; j < S * S / NT; ++j) info[j] = __ldg(P.cell_info + tid + j * NT);
+    int b = (int)(g0 - (long long)unit * P.nb);
+    const int first_unit = unit;
+    int seg_begin = b;
+    PrefetchSlots ps;
+    prefetch_init<NT>(P, tid, ps);
+    uint32_t wlo[MAXW], whi[MAXW];
+    prefetch_batch<NT>(P, ps, unit / Q, b, wlo, whi);
+    unpack_batch(P, ps, E, wlo, whi, unit / Q);
+    cta_sync();
+
+    // the batch whose MMAs are in flight: its epilogue (and its unit's flush) happen one iteration later
+    bool pend = false, pend_flush = false, pend_complete = false;
+    int pend_unit = 0, pend_slot = 0;
+    uint32_t phase = 0u;
+    auto retire = [&]() {
+      if constexpr (EPI) {
+        mbar_wait(&bar, phase);
+        phase ^= 1u;
+        tc_fence_after_sync();
+        tc_epilogue<NPROD>(tlane, acc);
+        if (pend_flush) flush(pend_unit, pend_complete, pend_slot);
+        tc_fence_before_sync();
+      }
+      pend = false;
+    };
+
+    const int ntask = F * P.R * 2;
+    for (long long g = g0; g < g1; ++g) {
+      int unit_n = unit, b_n = b + 1;
+      if (b_n == P.nb) { b_n = 0; ++unit_n; }
+      const bool more = g + 1 < g1;
+      if (more) prefetch_batch<NT>(P, ps, unit_n / Q, b_n, wlo, whi);
+
+      gather_batch<NT, DELTA>(P, E, gh, info);
+      cta_sync();
+
+      if constexpr (!EPI) {
+        const int l2 = unit % Q;
+        for (int base = warp * 32; base < ntask; base += TC_NT - TC_EPI_NT) {
+          const int task = base + lane;
+          const bool valid = task < ntask;
+          int f = 0, y = S - 1, h = 0;
+          if (valid) { h = task & 1; const int p = task >> 1; f = p / P.R; y = p - f * P.R; }
+          row_task<NB>(gh + f * PLANE + y * HS, tws + (l2 + Q * h) * TWV, h, valid);
+        }
+      } else {
+        if (pend) retire();  // the previous batch: D -> products -> registers; frees D for the next MMAs
+      }
+      pend = false;
+      cta_sync();
+
+      if (more) unpack_batch(P, ps, E, wlo, whi, unit_n / Q);  // E was last read by this batch's gather
+      tc_convert(gh, sB, tid);                                  // B was last read by the MMAs retired above
+      fence_smem_to_async_proxy();
+      cta_sync();  // B complete; gh is free for the next gather
+      if (tid == 0) {
+        tc_fence_after_sync();
+        tc_issue(sA_u, sB_u, tbase, &bar);
+      }
+      pend = true;
+      pend_unit = unit;
+      pend_flush = unit_n != unit || !more;
+      pend_complete = seg_begin == 0 && b == P.nb - 1;
+      pend_slot = unit == first_unit ? 0 : 1;
+      if (pend_flush) seg_begin = 0;
+      unit = unit_n; b = b_n;
     }
+    if (pend) retire();
   };
-
-  int b = (int)(g0 - (long long)unit * P.nb);
-  const int first_unit = unit;
-  int seg_begin = b;
-  PrefetchSlots ps;
-  prefetch_init<NT>(P, tid, ps);
-  uint32_t wlo[MAXW], whi[MAXW];
-  prefetch_batch<NT>(P, ps, unit / Q, b, wlo, whi);
-  unpack_batch(P, ps, E, wlo, whi, unit / Q);
-  __syncthreads();
-
-  // the batch whose MMAs are in flight: its epilogue (and its unit's flush) happen one iteration later
-  bool pend = false, pend_flush = false, pend_complete = false;
-  int pend_unit = 0, pend_slot = 0;
-  uint32_t phase = 0u;
-  auto retire = [&]() {
-    mbar_wait(&bar, phase);
-    phase ^= 1u;
-    tc_fence_after_sync();
-    tc_epilogue<NPROD>(tlane, acc);
-    if (pend_flush) flush(pend_unit, pend_complete, pend_slot);
-    pend = false;
-  };
-
-  const int ntask = F * P.R * 2;
-  for (long long g = g0; g < g1; ++g) {
-    int unit_n = unit, b_n = b + 1;
-    if (b_n == P.nb) { b_n = 0; ++unit_n; }
-    const bool more = g + 1 < g1;
-    if (more) prefetch_batch<NT>(P, ps, unit_n / Q, b_n, wlo, whi);
-
-    gather_batch<NT, DELTA>(P, E, gh, info);
-    __syncthreads();
-
-    const int l2 = unit % Q;
-    for (int base = warp * 32; base < ntask; base += NT) {
-      const int task = base + lane;
-      const bool valid = task < ntask;
-      int f = 0, y = S - 1, h = 0;
-      if (valid) { h = task & 1; const int p = task >> 1; f = p / P.R; y = p - f * P.R; }
-      row_task<NB>(gh + f * PLANE + y * HS, tws + (l2 + Q * h) * TWV, h, valid);
-    }
-    __syncthreads();
-
-    if (more) unpack_batch(P, ps, E, wlo, whi, unit_n / Q);  // E was last read by this batch's gather
-    if (pend) retire();            // the previous batch: D -> products -> registers; frees D and the B operands
-    tc_convert(gh, sB, tid);
-    fence_smem_to_async_proxy();
-    tc_fence_before_sync();
-    __syncthreads();               // B complete, every thread done reading D; gh is free for the next gather
-    if (tid == 0) {
-      tc_fence_after_sync();
-      tc_issue(sA_u, sB_u, tbase, &bar);
-    }
-    pend = true;
-    pend_unit = unit;
-    pend_flush = unit_n != unit || !more;
-    pend_complete = seg_begin == 0 && b == P.nb - 1;
-    pend_slot = unit == first_unit ? 0 : 1;
-    if (pend_flush) seg_begin = 0;
-    unit = unit_n; b = b_n;
-  }
-  if (pend) retire();
+  if (warp < (TC_NT - TC_EPI_NT) / 32) run(std::false_type{});
+  else run(std::true_type{});
   tmem_free_cta<512>(tbase, warp);
 }
 
@@ -897,9 +934,9 @@ static int launch_tc(const epic_plan* p, const FusedParams& P, const uint4* a_ta
   EPIC_CUDA_TRY(cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int grid = (int)std::min<long long>(P.total, p->n_sm);  // one CTA per SM (shared memory, all of TMEM)
   constexpr int NACC = NPROD == 4 ? 4 : 2;
-  if ((size_t)grid * 2 * NACC * 16 * TC_NT * sizeof(float) > p->scratch_bytes) return EPIC_ERR_RANGE;
+  if ((size_t)grid * 2 * NACC * TC_KPT * TC_EPI_NT * sizeof(float) > p->scratch_bytes) return EPIC_ERR_RANGE;
   kern<<<grid, TC_NT, smem, s>>>(P, a_tab);
-  epic_fused_fixup<4, NPROD, true><<<(unsigned)(P.total / P.nb), TC_NT, 0, s>>>(P, grid);
+  epic_fused_fixup<4, NPROD, true><<<(unsigned)(P.total / P.nb), TC_EPI_NT, 0, s>>>(P, grid);
   EPIC_CUDA_TRY(cudaGetLastError());
   return EPIC_OK;
 }
