@@ -332,6 +332,19 @@ def run_epic(args, wl):
         "gpu_launches": int(launches),
         "clocks": clocks,
     }
+    if path == 4:
+        # the tensor-core variant, reported beside the FP32 roofline above (same algorithmic flops, so the two
+        # paths compare directly): what its MMAs execute, against the measured dense BF16 peak of this pool
+        per_frame = 24 * 2.0 * 128 * 256 * 16 * (wl.N // 32) / 4   # 24 MMAs of 128x256x16 per (4 frames, one residue)
+        exe = per_frame * wl.frames / (kernel_ms * 1e-3) / 1e12
+        try:
+            bf16_peak = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["bf16_tflops_sustained"])
+            kind = "MEASURED_PEAKS.json bf16_tflops_sustained"
+        except (OSError, ValueError, KeyError):
+            bf16_peak, kind = 2250.0, "nominal dense BF16 (B200_PROFILING.md fallback)"
+        line["roofline"]["tensor"] = {"executed_bf16_tflops": exe, "peak": bf16_peak, "frac": exe / bf16_peak,
+                                      "peak_kind": kind, "executed_mma_flops_per_frame": per_frame,
+                                      "note": "BF16 hi/lo split: 3 products per real product, 4 real per complex"}
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(wl, volt, args.cpu_channels, args.input_order.upper())
     print(json.dumps(line))
