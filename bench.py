@@ -155,6 +155,8 @@ def run_reference(args, wl):
         return
     n_t = min(wl.n_t, 250)
     small = make_config(wl.index, n_chan=2, n_t=n_t)
+    if wl.ant_uv.ndim == 3:
+        small = per_channel_variant(small)
     volt = small.voltages()
     times = []
     res = None

@@ -90,3 +90,17 @@ def test_multi_rank_reduction_and_sharding_on_gloo(tmp_path):
     outs = [p.communicate(timeout=120)[0] for p in procs]
     for p, o in zip(procs, outs):
         assert p.returncode == 0, o
+
+
+def test_bench_per_channel_variant_keeps_the_configs_shape():
+    import bench
+    from workloads import make_config
+    base = make_config(3, n_chan=4, n_t=6)
+    pc = bench.per_channel_variant(base)
+    assert pc.ant_uv.shape == (4, 256, 2) and pc.taps.shape == (4, 256, 3, 3, 2)
+    assert (pc.grid_n, pc.pad, pc.n_pol, pc.n_products, pc.n_t, pc.index) == (64, 2, 2, 4, 6, 3)
+    # 25 kHz channels from 38 MHz: coordinates relative to the centre grow by 25/38000 per channel
+    off = pc.ant_uv.astype(np.float64) - 32.0
+    np.testing.assert_allclose(off[3], off[0] * (38e6 + 75e3) / 38e6, rtol=1e-4, atol=1e-4)
+    assert bench.algorithmic_flops_per_frame(pc) == bench.algorithmic_flops_per_frame(base)
+    assert pc.voltages().shape == (6, 4, 2, 256)
