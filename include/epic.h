@@ -14,7 +14,9 @@
  *
  * N = grid_n * pad (zero-padded plane side, a power of two).  The transform is the
  * unnormalised inverse DFT in natural order with zenith (l = m = 0) at [0][0]; no fftshift.
- * All arithmetic is fp32 (the paper's complex64).
+ * All arithmetic is fp32 (the paper's complex64); the optional EPIC_PATH_TENSOR
+ * forms the column transform from BF16 hi + lo split operands with fp32 accumulation, to the
+ * same tolerance.
  *
  * Conventions.  Every function returns EPIC_OK (0) or a negative epic_status; nothing throws
  * across the ABI.  Argument validation is synchronous.  Device work is enqueued on `stream`
