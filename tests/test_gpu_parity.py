@@ -553,3 +553,18 @@ def test_tensor_core_path_is_bit_reproducible_and_rejected_where_unsupported():
     with epic.Plan(small.grid_n, small.pad, small.ant_uv, small.taps, small.kernel_k) as plan:
         with pytest.raises(epic.EpicError):
             plan.set_path(epic.EPIC_PATH_TENSOR)
+
+
+def test_tensor_core_path_full_size_c2_sampled_channels():
+    """C2 at full extent through EPIC_PATH_TENSOR, the launch configuration `bench.py --path tensor`
+    times (one call, 148 CTAs); whole channels against the oracle, properties for the rest."""
+    wl = make_config(2)
+    v = wl.voltages()
+    gpu, info = run_gpu(wl, volt=v, path=4, return_plan_info=True)
+    assert info["path"] == 4 and info["launches"] == 2
+    channels = [0, 63, 127]
+    ref = run_oracle(wl, volt=v, channels=channels)
+    assert_parity(gpu[channels], ref, what=f"{wl.name} tensor path, channels {channels}")
+    assert np.isfinite(gpu).all() and (gpu >= 0).all()
+    totals = gpu[:, 0].sum(axis=(1, 2))
+    assert totals.min() > 0.5 * totals.max()
