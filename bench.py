@@ -305,10 +305,13 @@ def run_epic(args, wl):
     kernel_ms = float(np.mean(dev_ms))           # rank 0's own kernel time (one launch per step when fused)
     achieved = flops * wl.frames / (kernel_ms * 1e-3) / 1e12
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")   # measured DRAM bytes per launch (profiles/traffic.md)
     if os.path.exists(tpath):
         try:
-            traffic = json.load(open(tpath)).get(f"{wl.name}:{PATH_NAMES.get(path)}")
+            with open(tpath) as fh:
+                rows = dict(ln.strip().split(",")[:2] for ln in fh.read().splitlines()[1:] if "," in ln)
+            key = f"{wl.name}:{PATH_NAMES.get(path)}"
+            traffic = int(rows[key]) if key in rows else None
         except (OSError, ValueError):
             traffic = None
     line = {
