@@ -370,7 +370,7 @@ def main():
     ap.add_argument("--n-chan", type=int, default=None)
     ap.add_argument("--n-t", type=int, default=None)
     ap.add_argument("--n-ant", type=int, default=None)
-    ap.add_argument("--cpu-channels", type=int, default=8)
+    ap.add_argument("--cpu-channels", type=int, default=16, help="channels of the workload the oracle images for cpu_baseline (~13 s on C2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--input-order", default="tcpa", choices=["tcpa", "tcap"], help="tcap = [T][C][A][Np], transposed in the load")
     ap.add_argument("--delay-phasors", action="store_true", help="apply per-(channel, pol, antenna) delay phasors")
