@@ -353,7 +353,9 @@ def run_epic(args, wl):
                                       "peak_kind": kind, "executed_mma_flops_per_frame": per_frame,
                                       "note": "BF16 hi/lo split: 3 products per real product, 4 real per complex"}
     if world == 1 and not args.no_cpu_baseline:
-        line["cpu_baseline"] = cpu_baseline(wl, volt, args.cpu_channels, args.input_order.upper())
+        # bounded sample: the oracle's cost per frame grows with the plane (N^2 log N), so fewer channels of the big configs
+        n_cpu = max(1, args.cpu_channels * (128 * 128) // max(128 * 128, wl.N * wl.N * wl.n_planes // 2))
+        line["cpu_baseline"] = cpu_baseline(wl, volt, n_cpu, args.input_order.upper())
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
