@@ -104,6 +104,7 @@ struct FusedParams {
   int native;                // input order [T][C][A][Np] instead of [T][C][Np][A]
   const float4* phasor;      // delay phasors, pair-packed [C][A], or nullptr
   int n_t, n_chan, n_ant, n_pol, n_planes;
+  int n_ent;                 // gather entries (one layout)
   int R, Cc;                 // occupied rows / columns of the block
   int nb;                    // batches per unit
   long long total;           // n_chan * Q * nb batches in all
@@ -167,9 +168,11 @@ __device__ __forceinline__ void unpack_batch(const FusedParams& P, const Prefetc
 // gather lists, in table order, for all F pair-planes (collisions sum).  The
 // list holds every cell of the R x 32 block (empty ones are written as zeros) sorted by entry
 // count, so the 32 cells of a warp have (nearly) equal trip counts.
-template <int NT, bool DELTA>
+template <int NT, bool DELTA, bool STG = false>
 __device__ __forceinline__ void gather_batch(const FusedParams& P, const float4* __restrict__ E,
-                                             float4* __restrict__ gh, const uint2 (&info)[S * S / NT]) {
+                                             float4* __restrict__ gh, const uint2 (&info)[S * S / NT],
+                                             const uint16_t* __restrict__ ant_s = nullptr,
+                                             const float2* __restrict__ tap_s = nullptr) {
 #pragma unroll
   for (int j = 0; j < S * S / NT; ++j) {
     if (info[j].y == 0xFFFFFFFFu) continue;
@@ -178,7 +181,7 @@ __device__ __forceinline__ void gather_batch(const FusedParams& P, const float4*
 #pragma unroll
     for (int f = 0; f < F; ++f) { sr[f] = make_float2(0.0f, 0.0f); si[f] = make_float2(0.0f, 0.0f); }
     for (uint32_t e = beg; e < beg + cnt; ++e) {
-      const float4* ea = E + __ldg(P.ent_ant + e);
+      const float4* ea = E + (STG ? (uint32_t)ant_s[e] : (uint32_t)__ldg(P.ent_ant + e));
       if (DELTA) {
 #pragma unroll
         for (int f = 0; f < F; ++f) {
@@ -187,7 +190,7 @@ __device__ __forceinline__ void gather_batch(const FusedParams& P, const float4*
           si[f] = __fadd2_rn(si[f], make_float2(v.z, v.w));
         }
       } else {
-        const float2 w = __ldg(P.ent_tap + e);
+        const float2 w = STG ? tap_s[e] : __ldg(P.ent_tap + e);
         const float2 wr = f2(w.x), wi = f2(w.y);
 #pragma unroll
         for (int f = 0; f < F; ++f) {
@@ -315,9 +318,13 @@ __device__ __forceinline__ void col_task_tmem(const float4* __restrict__ col, co
 
 // PC: every channel has its own cell table (per-channel plans); a separate instantiation, because
 // making the cell records loop-variant costs the one-layout kernels 1-2 % (measured).
-template <int Q, int NPROD, bool DELTA, int NB, bool PC>
+// STG: the gather's (antenna, tap) tables are copied to shared memory once per CTA (tap kernels of
+// one-layout plans whose tables fit beside two resident CTAs): their reads leave the L1/L2 path,
+// C3 +2.8 % (measured); the delta kernels, whose table is 2 bytes per antenna, gain nothing.
+template <int Q, int NPROD, bool DELTA, int NB, bool PC, bool STG>
 __global__ void __launch_bounds__(64 * Q, 2)
 epic_fused_kernel(FusedParams P) {
+  static_assert(!(STG && (DELTA || PC)), "staged tables: tap kernels of one-layout plans only");
   constexpr int NT = 64 * Q, N = 32 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* gh = reinterpret_cast<float4*>(smem_raw);  // [F][32][HS]
@@ -339,6 +346,11 @@ epic_fused_kernel(FusedParams P) {
     info[j] = __ldg(P.cell_info + (PC ? (size_t)(unit / Q) * (S * S) : (size_t)0) + tid + j * NT);
   for (int i = tid; i < F * PLANE; i += NT) gh[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);  // rows >= R stay zero
   for (int i = tid; i < 2 * Q * TWV; i += NT) tws[i] = __ldg(P.tw + i);
+  float2* tap_s = reinterpret_cast<float2*>(E + F * P.n_ant);       // [n_ent] (STG only)
+  uint16_t* ant_s = reinterpret_cast<uint16_t*>(tap_s + P.n_ent);   // [n_ent]
+  if constexpr (STG) {
+    for (int i = tid; i < P.n_ent; i += NT) { tap_s[i] = __ldg(P.ent_tap + i); ant_s[i] = __ldg(P.ent_ant + i); }
+  }
   __syncthreads();
 
   // column role: 16 consecutive l1 x 2 residues per warp, the two residues of a column in ADJACENT
@@ -431,7 +443,7 @@ epic_fused_kernel(FusedParams P) {
     const bool more = g + 1 < g1;
     if (more) prefetch_batch<NT>(P, ps, unit_n / Q, b_n, wlo, whi);
 
-    gather_batch<NT, DELTA>(P, E, gh, info);
+    gather_batch<NT, DELTA, STG>(P, E, gh, info, ant_s, tap_s);
     __syncthreads();
 
     const int l2 = unit % Q;
@@ -741,11 +753,13 @@ size_t fused_smem_bytes(int n_ant) {
   return ((size_t)F * PLANE + (size_t)2 * Q * TWV + (size_t)F * n_ant) * sizeof(float4);
 }
 
-template <int Q, int NPROD, bool DELTA, int NB, bool PC>
+inline size_t fused_stage_bytes(int n_ent) { return ((size_t)n_ent * (sizeof(float2) + sizeof(uint16_t)) + 15) & ~(size_t)15; }
+
+template <int Q, int NPROD, bool DELTA, int NB, bool PC, bool STG = false>
 int launch_fused(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
   constexpr int NT = 64 * Q;
-  const size_t smem = fused_smem_bytes<Q>(P.n_ant);
-  auto kern = epic_fused_kernel<Q, NPROD, DELTA, NB, PC>;
+  const size_t smem = fused_smem_bytes<Q>(P.n_ant) + (STG ? fused_stage_bytes(P.n_ent) : 0);
+  auto kern = epic_fused_kernel<Q, NPROD, DELTA, NB, PC, STG>;
   if (smem > 48 * 1024)
     EPIC_CUDA_TRY(cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int per_sm = 0;
@@ -769,8 +783,13 @@ int launch_fused(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
 template <int Q, int NPROD, bool DELTA>
 int launch_fused_nb(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
   // elements y + 16 of a row/column are read only while y < NB (the rest of the block is empty)
-  const bool pc = P.cell_stride != 0;
-  if (std::max(p->R, p->Cc) <= 16 + 12)
+  const bool pc = P.cell_stride != 0, nb12 = std::max(p->R, p->Cc) <= 16 + 12;
+  if constexpr (!DELTA) {  // staged gather tables, if two CTAs still fit an SM with them
+    if (!pc && 2 * (fused_smem_bytes<Q>(P.n_ant) + fused_stage_bytes(P.n_ent) + 1024 + 128) <= (size_t)227 * 1024)
+      return nb12 ? launch_fused<Q, NPROD, DELTA, 12, false, true>(p, P, s)
+                  : launch_fused<Q, NPROD, DELTA, 16, false, true>(p, P, s);
+  }
+  if (nb12)
     return pc ? launch_fused<Q, NPROD, DELTA, 12, true>(p, P, s) : launch_fused<Q, NPROD, DELTA, 12, false>(p, P, s);
   return pc ? launch_fused<Q, NPROD, DELTA, 16, true>(p, P, s) : launch_fused<Q, NPROD, DELTA, 16, false>(p, P, s);
 }
@@ -779,7 +798,7 @@ template <int Q>
 int launch_fused_q(const epic_plan* p, const FusedParams& P, int n_products, cudaStream_t s) {
   const bool delta = p->t.is_delta != 0;
 #ifdef EPIC_FUSED_DEV_ONE  // development builds: compile a single instantiation
-  if (Q == 4 && n_products == 2 && delta) return launch_fused<4, 2, true, 12, false>(p, P, s);
+  if (Q == 4 && n_products == 2 && delta) return launch_fused<4, 2, true, 12, false, false>(p, P, s);
   return EPIC_ERR_RANGE;
 #else
   switch (n_products) {
@@ -957,6 +976,7 @@ static void fill_params(const epic_plan* p, const ImageArgs& a, FusedParams& P) 
   P.n_t = a.n_t;
   P.n_chan = a.n_chan;
   P.n_ant = p->n_ant;
+  P.n_ent = p->t.n_ent;
   P.n_pol = a.n_pol;
   P.n_planes = a.n_planes;
   P.R = p->R;

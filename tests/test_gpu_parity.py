@@ -134,6 +134,8 @@ FUSED_CAPABLE = [
     make_custom(grid_n=32, pad=2, n_ant=40, n_pol=1, kernel_k=3, n_chan=3, n_t=16, layout="disc"),
     make_custom(grid_n=64, pad=2, n_ant=512, n_pol=2, kernel_k=1, n_chan=2, n_t=5, layout="disc"),  # 2 prefetch slots
     make_custom(grid_n=32, pad=4, n_ant=100, n_pol=2, kernel_k=5, n_chan=2, n_t=7, layout="disc", n_products=4),
+    make_custom(grid_n=64, pad=2, n_ant=256, n_pol=2, kernel_k=5, n_chan=2, n_t=6, layout="disc", n_products=2,
+                seed=21),                                  # 6400 gather entries: too many to stage in shared memory
 ]
 
 
