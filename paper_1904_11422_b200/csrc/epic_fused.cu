@@ -154,9 +154,18 @@ __device__ __forceinline__ void prefetch_batch(const FusedParams& P, const Prefe
   }
 }
 
-// registers -> E[F][A] (float4 per antenna), S1
+// registers -> E[F][A] (float4 per antenna), S1.  EB: E holds one 32-bit word per antenna instead, the four
+// values as bytes biased by 8 (epic_packed.cuh), for the integer gather of the delta kernels.
+template <bool EB = false>
 __device__ __forceinline__ void unpack_batch(const FusedParams& P, const PrefetchSlots& ps, float4* __restrict__ E,
                                              const uint32_t (&wlo)[MAXW], const uint32_t (&whi)[MAXW], int c) {
+  if constexpr (EB) {
+    uint32_t* Eb = reinterpret_cast<uint32_t*>(E);
+#pragma unroll
+    for (int k = 0; k < MAXW; ++k)
+      if (ps.j[k] >= 0) *reinterpret_cast<uint4*>(Eb + ps.j[k] * P.n_ant + ps.a[k]) = unpack_words_b8(wlo[k], whi[k]);
+    return;
+  }
 #pragma unroll
   for (int k = 0; k < MAXW; ++k)
     if (ps.j[k] >= 0)
@@ -168,7 +177,10 @@ __device__ __forceinline__ void unpack_batch(const FusedParams& P, const Prefetc
 // gather lists, in table order, for all F pair-planes (collisions sum).  The
 // list holds every cell of the R x 32 block (empty ones are written as zeros) sorted by entry
 // count, so the 32 cells of a warp have (nearly) equal trip counts.
-template <int NT, bool DELTA, bool STG = false>
+// EB (delta kernel, at most 16 antennas per cell, no delay phasors): the four values of an antenna
+// are bytes 0..15 of one word, so a cell's sum is ONE integer add per antenna and pair -- the byte
+// sums stay below 256 -- turned into floats once per cell: exact, like the float adds it replaces.
+template <int NT, bool DELTA, bool STG = false, bool EB = false>
 __device__ __forceinline__ void gather_batch(const FusedParams& P, const float4* __restrict__ E,
                                              float4* __restrict__ gh, const uint2 (&info)[S * S / NT],
                                              const uint16_t* __restrict__ ant_s = nullptr,
@@ -177,6 +189,26 @@ __device__ __forceinline__ void gather_batch(const FusedParams& P, const float4*
   for (int j = 0; j < S * S / NT; ++j) {
     if (info[j].y == 0xFFFFFFFFu) continue;
     const uint32_t beg = info[j].x >> 8, cnt = info[j].x & 0xFFu;
+    if constexpr (EB) {
+      const uint32_t* Eb = reinterpret_cast<const uint32_t*>(E);
+      uint32_t sum[F];
+#pragma unroll
+      for (int f = 0; f < F; ++f) sum[f] = 0u;
+      for (uint32_t e = beg; e < beg + cnt; ++e) {
+        const uint32_t* ea = Eb + __ldg(P.ent_ant + e);
+#pragma unroll
+        for (int f = 0; f < F; ++f) sum[f] += ea[f * P.n_ant];
+      }
+      const float2 bias = f2(-(12582912.0f + 8.0f * (float)cnt));  // mantissa trick of epic_packed.cuh, cnt biases of 8
+      float4* dst = gh + info[j].y;
+#pragma unroll
+      for (int f = 0; f < F; ++f) {
+        const float2 vr = __fadd2_rn(make_float2(biased_byte_to_float_bits(sum[f], 0), biased_byte_to_float_bits(sum[f], 1)), bias);
+        const float2 vi = __fadd2_rn(make_float2(biased_byte_to_float_bits(sum[f], 2), biased_byte_to_float_bits(sum[f], 3)), bias);
+        dst[f * PLANE] = make_float4(vr.x, vr.y, vi.x, vi.y);
+      }
+      continue;
+    }
     float2 sr[F], si[F];
 #pragma unroll
     for (int f = 0; f < F; ++f) { sr[f] = make_float2(0.0f, 0.0f); si[f] = make_float2(0.0f, 0.0f); }
@@ -433,7 +465,7 @@ epic_fused_kernel(FusedParams P) {
   prefetch_init<NT>(P, tid, ps);
   uint32_t wlo[MAXW], whi[MAXW];
   prefetch_batch<NT>(P, ps, unit / Q, b, wlo, whi);
-  unpack_batch(P, ps, E, wlo, whi, unit / Q);
+  unpack_batch<DELTA>(P, ps, E, wlo, whi, unit / Q);
   __syncthreads();
 
   const int ntask = F * P.R * 2;
@@ -443,7 +475,7 @@ epic_fused_kernel(FusedParams P) {
     const bool more = g + 1 < g1;
     if (more) prefetch_batch<NT>(P, ps, unit_n / Q, b_n, wlo, whi);
 
-    gather_batch<NT, DELTA, STG>(P, E, gh, info, ant_s, tap_s);
+    gather_batch<NT, DELTA, STG, DELTA>(P, E, gh, info, ant_s, tap_s);
     __syncthreads();
 
     const int l2 = unit % Q;
@@ -457,7 +489,7 @@ epic_fused_kernel(FusedParams P) {
     }
     __syncthreads();
 
-    if (more) unpack_batch(P, ps, E, wlo, whi, unit_n / Q);  // E was last read by this batch's gather
+    if (more) unpack_batch<DELTA>(P, ps, E, wlo, whi, unit_n / Q);  // E was last read by this batch's gather
 #pragma unroll 1
     for (int f = 0; f < F; ++f) {
       // launder the table offset: the twiddles are re-read per task, not held in 18 registers
@@ -746,6 +778,7 @@ struct FusedTables {
   uint2* cell_info;
   float4* tw;
   uint4* a_tab;  // tensor-core path: the DFT matrix as BF16 hi/lo operands (Q = 4 only), or nullptr
+  uint32_t max_cnt;  // most gather entries in one cell
 };
 
 template <int Q>
@@ -796,7 +829,10 @@ int launch_fused_nb(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
 
 template <int Q>
 int launch_fused_q(const epic_plan* p, const FusedParams& P, int n_products, cudaStream_t s) {
-  const bool delta = p->t.is_delta != 0;
+  // The delta instantiations gather in integers (gather_batch EB): no delay phasors, at most 16 antennas
+  // in a cell.  Other delta plans run the tap kernels with their unit taps (1 + 0i), which is exact too.
+  const FusedTables* ft = static_cast<const FusedTables*>(p->d_fused);
+  const bool delta = p->t.is_delta != 0 && P.phasor == nullptr && ft->max_cnt <= 16u;
 #ifdef EPIC_FUSED_DEV_ONE  // development builds: compile a single instantiation
   if (Q == 4 && n_products == 2 && delta) return launch_fused<4, 2, true, 12, false, false>(p, P, s);
   return EPIC_ERR_RANGE;
@@ -889,6 +925,8 @@ int fused_plan_init(epic_plan* p) {
   ft->cell_info = nullptr;
   ft->tw = nullptr;
   ft->a_tab = nullptr;
+  ft->max_cnt = 0;
+  for (const CellRec& c : p->h_cells) ft->max_cnt = std::max(ft->max_cnt, c.ent_count);
   cudaError_t ce = cudaMalloc(&ft->cell_info, info.size() * sizeof(uint2));
   if (ce == cudaSuccess) ce = cudaMalloc(&ft->tw, tw.size() * sizeof(float4));
   if (ce == cudaSuccess && !a_tab.empty()) {
