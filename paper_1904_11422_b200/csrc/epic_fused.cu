@@ -707,7 +707,7 @@ __global__ void __launch_bounds__(TC_NT, 1) epic_tc_kernel(FusedParams P, const 
     prefetch_init<NT>(P, tid, ps);
     uint32_t wlo[MAXW], whi[MAXW];
     prefetch_batch<NT>(P, ps, unit / Q, b, wlo, whi);
-    unpack_batch(P, ps, E, wlo, whi, unit / Q);
+    unpack_batch<DELTA>(P, ps, E, wlo, whi, unit / Q);
     cta_sync();
 
     // the batch whose MMAs are in flight: its epilogue (and its unit's flush) happen one iteration later
@@ -733,7 +733,7 @@ __global__ void __launch_bounds__(TC_NT, 1) epic_tc_kernel(FusedParams P, const 
       const bool more = g + 1 < g1;
       if (more) prefetch_batch<NT>(P, ps, unit_n / Q, b_n, wlo, whi);
 
-      gather_batch<NT, DELTA>(P, E, gh, info);
+      gather_batch<NT, DELTA, false, DELTA>(P, E, gh, info);
       cta_sync();
 
       if constexpr (!EPI) {
@@ -751,7 +751,7 @@ __global__ void __launch_bounds__(TC_NT, 1) epic_tc_kernel(FusedParams P, const 
       pend = false;
       cta_sync();
 
-      if (more) unpack_batch(P, ps, E, wlo, whi, unit_n / Q);  // E was last read by this batch's gather
+      if (more) unpack_batch<DELTA>(P, ps, E, wlo, whi, unit_n / Q);  // E was last read by this batch's gather
       tc_convert(gh, sB, tid);                                  // B was last read by the MMAs retired above
       fence_smem_to_async_proxy();
       cta_sync();  // B complete; gh is free for the next gather
@@ -1028,7 +1028,9 @@ int tensor_image(epic_plan* p, const ImageArgs& a) {
   const FusedTables* ft = static_cast<const FusedTables*>(p->d_fused);
   FusedParams P;
   fill_params(p, a, P);
-  const bool delta = p->t.is_delta != 0, nb12 = std::max(p->R, p->Cc) <= 16 + 12;
+  // delta instantiations: integer gather, under the conditions of launch_fused_q
+  const bool delta = p->t.is_delta != 0 && P.phasor == nullptr && ft->max_cnt <= 16u;
+  const bool nb12 = std::max(p->R, p->Cc) <= 16 + 12;
   int st;
 #define EPIC_TC_CASE(NPROD, DELTA, NB) st = launch_tc<NPROD, DELTA, NB>(p, P, ft->a_tab, a.stream)
   if (a.n_products == 2) {
