@@ -44,6 +44,54 @@ struct Entry {
   int ant, tap;  // tap = iy*K + ix
 };
 
+// Entry order inside a cell, chosen for the fused kernel's gather (epic_fused.cu, gather_batch):
+// a quarter-warp owns 8 consecutive cells of the count-sorted slot list and step i of its loop
+// reads entry i of each cell with one LDS.128 of E[antenna]; that load is conflict-free when
+// the 8 antennas differ mod 8 (16-byte bank groups) or coincide (broadcast).  Greedy, per group
+// and step: each cell takes the remaining entry whose bank group holds the fewest other antennas
+// so far.  Only the order of a cell's sum changes (rounding order; PAPER.md:122-124 fixes none).
+static void bank_order_entries(epic_plan* p, size_t cell0) {
+  constexpr int S = 32, G = 8;
+  std::vector<const CellRec*> dense((size_t)S * S, nullptr);
+  for (size_t i = cell0; i < p->h_cells.size(); ++i) {
+    const CellRec& c = p->h_cells[i];
+    dense[(size_t)c.y * S + c.x] = &c;
+  }
+  std::vector<const CellRec*> li;  // the slot order of fused_plan_init: descending count, stable in (y, x)
+  for (int y = 0; y < p->R; ++y)
+    for (int x = 0; x < S; ++x) li.push_back(dense[(size_t)y * S + x]);
+  auto count_of = [](const CellRec* c) { return c ? c->ent_count : 0u; };
+  std::stable_sort(li.begin(), li.end(),
+                   [&](const CellRec* a, const CellRec* b) { return count_of(a) > count_of(b); });
+  for (size_t g = 0; g < li.size(); g += G) {
+    const uint32_t steps = count_of(li[g]);
+    if (steps < 2) break;  // nothing left to choose
+    for (uint32_t step = 0; step < steps; ++step) {
+      std::vector<uint16_t> in_bank[G];
+      for (size_t lane = g; lane < std::min(li.size(), g + G); ++lane) {
+        const CellRec* c = li[lane];
+        if (step >= count_of(c)) continue;
+        uint32_t best = step;
+        size_t best_cost = ~(size_t)0;
+        for (uint32_t r = step; r < c->ent_count; ++r) {
+          const uint16_t ant = p->h_ent_ant[c->ent_begin + r];
+          const std::vector<uint16_t>& b = in_bank[ant % G];
+          const size_t cost = std::find(b.begin(), b.end(), ant) != b.end() ? 0 : b.size();
+          if (cost < best_cost) {
+            best_cost = cost;
+            best = r;
+          }
+        }
+        std::swap(p->h_ent_ant[c->ent_begin + step], p->h_ent_ant[c->ent_begin + best]);
+        std::swap(p->h_ent_tap[c->ent_begin + step], p->h_ent_tap[c->ent_begin + best]);
+        const uint16_t ant = p->h_ent_ant[c->ent_begin + step];
+        std::vector<uint16_t>& b = in_bank[ant % G];
+        if (std::find(b.begin(), b.end(), ant) == b.end()) b.push_back(ant);
+      }
+    }
+  }
+}
+
 static int build_tables(epic_plan* p, const float* ant_uv_all, const float* taps_all) {
   const int N = p->N, K = p->K, A = p->n_ant, h = (K - 1) / 2, L = p->n_layout;
   const size_t per_layout = (size_t)A * K * K;
@@ -118,6 +166,7 @@ static int build_tables(epic_plan* p, const float* ant_uv_all, const float* taps
       }
       p->h_ent_tap[ent0 + i] = w;
     }
+    if (taps && p->R <= 32 && p->Cc <= 32) bank_order_entries(p, cell0);
     rp[0] = (uint32_t)cell0;  // indices into the concatenated cells array
     for (int y = 0; y < p->R; ++y) rp[y + 1] += rp[y];
     p->h_cell_off.push_back((uint32_t)p->h_cells.size());
