@@ -866,11 +866,20 @@ int fused_plan_init(epic_plan* p) {
     }
     // every cell of the R x 32 block (columns >= Cc are re-zeroed each batch: the row pass writes
     // its output in place), sorted by entry count so that warps see uniform trip counts
+    // (tap plans: the plan builder has already chosen the order, bank-aware within equal counts)
     std::vector<uint2> li;
-    for (int y = 0; y < p->R; ++y)
-      for (int x = 0; x < S; ++x) li.push_back(make_uint2(dense[(size_t)y * S + x], (uint32_t)(y * HS + x)));
-    std::stable_sort(li.begin(), li.end(),
-                     [](const uint2& a, const uint2& b) { return (a.x & 0xFFu) > (b.x & 0xFFu); });
+    const size_t n_slots = (size_t)p->R * S;
+    if (p->h_slot_order.size() == (size_t)p->n_layout * n_slots) {
+      for (size_t i = 0; i < n_slots; ++i) {
+        const uint32_t s = p->h_slot_order[(size_t)l * n_slots + i], y = s / S, x = s % S;
+        li.push_back(make_uint2(dense[s], (uint32_t)(y * HS + x)));
+      }
+    } else {
+      for (int y = 0; y < p->R; ++y)
+        for (int x = 0; x < S; ++x) li.push_back(make_uint2(dense[(size_t)y * S + x], (uint32_t)(y * HS + x)));
+      std::stable_sort(li.begin(), li.end(),
+                       [](const uint2& a, const uint2& b) { return (a.x & 0xFFu) > (b.x & 0xFFu); });
+    }
     li.resize((size_t)S * S, make_uint2(0u, 0xFFFFFFFFu));
     info.insert(info.end(), li.begin(), li.end());
   }

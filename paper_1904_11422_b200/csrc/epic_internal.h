@@ -61,6 +61,8 @@ struct epic_plan {
   std::vector<uint32_t> h_cell_off;     // [n_layout + 1]: layout l's cells are [h_cell_off[l], h_cell_off[l+1])
   std::vector<uint16_t> h_ent_ant;
   std::vector<float2> h_ent_tap;
+  std::vector<uint16_t> h_slot_order;   // tap plans that fit 32x32: per layout, the fused kernel's slot list as
+                                        // cells y*32+x of the R x 32 block (bank_order_entries); else empty
 };
 
 namespace epic {

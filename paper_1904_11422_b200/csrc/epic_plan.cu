@@ -44,33 +44,77 @@ struct Entry {
   int ant, tap;  // tap = iy*K + ix
 };
 
-// Entry order inside a cell, chosen for the fused kernel's gather (epic_fused.cu, gather_batch):
-// a quarter-warp owns 8 consecutive cells of the count-sorted slot list and step i of its loop
-// reads entry i of each cell with one LDS.128 of E[antenna]; that load is conflict-free when
-// the 8 antennas differ mod 8 (16-byte bank groups) or coincide (broadcast).  Greedy, per group
-// and step: each cell takes the remaining entry whose bank group holds the fewest other antennas
-// so far.  Only the order of a cell's sum changes (rounding order; PAPER.md:122-124 fixes none).
+// Slot order and entry order for the fused kernel's gather (epic_fused.cu, gather_batch): a
+// quarter-warp owns 8 consecutive cells of the slot list (descending entry count, so that warps
+// see uniform trip counts) and step i of its loop reads entry i of each cell with one LDS.128 of
+// E[antenna]; that load is conflict-free when the 8 antennas differ mod 8 (16-byte bank groups)
+// or coincide (broadcast).  Two greedy passes at plan time: (1) among the next cells of equal
+// count, a group takes the one whose antennas share the fewest bank groups (and the most
+// antennas) with the group so far; (2) per group and step, each cell takes the remaining entry
+// whose bank group holds the fewest other antennas so far.  Only the order of a cell's sum
+// changes (rounding order; PAPER.md:122-124 fixes none).  Appends the layout's R*32 slots to
+// h_slot_order.
 static void bank_order_entries(epic_plan* p, size_t cell0) {
-  constexpr int S = 32, G = 8;
+  constexpr int S = 32, G = 8, WINDOW = 96;
   std::vector<const CellRec*> dense((size_t)S * S, nullptr);
   for (size_t i = cell0; i < p->h_cells.size(); ++i) {
     const CellRec& c = p->h_cells[i];
     dense[(size_t)c.y * S + c.x] = &c;
   }
-  std::vector<const CellRec*> li;  // the slot order of fused_plan_init: descending count, stable in (y, x)
+  auto count_of = [&](uint16_t s) { return dense[s] ? dense[s]->ent_count : 0u; };
+  std::vector<uint16_t> rest;  // descending count, stable in (y, x)
   for (int y = 0; y < p->R; ++y)
-    for (int x = 0; x < S; ++x) li.push_back(dense[(size_t)y * S + x]);
-  auto count_of = [](const CellRec* c) { return c ? c->ent_count : 0u; };
-  std::stable_sort(li.begin(), li.end(),
-                   [&](const CellRec* a, const CellRec* b) { return count_of(a) > count_of(b); });
-  for (size_t g = 0; g < li.size(); g += G) {
-    const uint32_t steps = count_of(li[g]);
-    if (steps < 2) break;  // nothing left to choose
+    for (int x = 0; x < S; ++x) rest.push_back((uint16_t)(y * S + x));
+  std::stable_sort(rest.begin(), rest.end(), [&](uint16_t a, uint16_t b) { return count_of(a) > count_of(b); });
+  // (1) groups of G slots
+  std::vector<uint16_t> order;
+  order.reserve(rest.size());
+  size_t head = 0;
+  std::vector<char> taken(rest.size(), 0);
+  while (order.size() < rest.size()) {
+    std::vector<uint16_t> grp_ants;
+    for (int lane = 0; lane < G && order.size() < rest.size(); ++lane) {
+      while (taken[head]) ++head;
+      const uint32_t cnt = count_of(rest[head]);
+      size_t pick = head;
+      if (cnt > 0 && !grp_ants.empty()) {
+        long best = 0;
+        bool have = false;
+        size_t seen = 0;
+        for (size_t i = head; i < rest.size() && seen < WINDOW; ++i) {
+          if (taken[i]) continue;
+          if (count_of(rest[i]) != cnt) break;
+          ++seen;
+          const CellRec* c = dense[rest[i]];
+          long cost = 0;
+          for (uint32_t r = 0; r < c->ent_count; ++r) {
+            const uint16_t ant = p->h_ent_ant[c->ent_begin + r];
+            for (uint16_t g : grp_ants) cost += (g == ant) ? -8 : ((g % G) == (ant % G) ? 1 : 0);
+          }
+          if (!have || cost < best) {
+            have = true;
+            best = cost;
+            pick = i;
+          }
+        }
+      }
+      taken[pick] = 1;
+      order.push_back(rest[pick]);
+      if (const CellRec* c = dense[rest[pick]])
+        for (uint32_t r = 0; r < c->ent_count; ++r) grp_ants.push_back(p->h_ent_ant[c->ent_begin + r]);
+    }
+  }
+  p->h_slot_order.insert(p->h_slot_order.end(), order.begin(), order.end());
+  // (2) entry order inside each cell
+  for (size_t g = 0; g < order.size(); g += G) {
+    uint32_t steps = 0;
+    for (size_t lane = g; lane < std::min(order.size(), g + G); ++lane) steps = std::max(steps, count_of(order[lane]));
+    if (steps == 0) break;
     for (uint32_t step = 0; step < steps; ++step) {
       std::vector<uint16_t> in_bank[G];
-      for (size_t lane = g; lane < std::min(li.size(), g + G); ++lane) {
-        const CellRec* c = li[lane];
-        if (step >= count_of(c)) continue;
+      for (size_t lane = g; lane < std::min(order.size(), g + G); ++lane) {
+        const CellRec* c = dense[order[lane]];
+        if (!c || step >= c->ent_count) continue;
         uint32_t best = step;
         size_t best_cost = ~(size_t)0;
         for (uint32_t r = step; r < c->ent_count; ++r) {
@@ -118,6 +162,7 @@ static int build_tables(epic_plan* p, const float* ant_uv_all, const float* taps
   circular_box(occ_x, N, &p->x0, &p->Cc);
 
   p->h_cells.clear();
+  p->h_slot_order.clear();
   p->h_cell_off.assign(1, 0u);
   p->h_ent_ant.resize((size_t)L * per_layout);
   p->h_ent_tap.resize((size_t)L * per_layout);
