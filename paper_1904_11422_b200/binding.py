@@ -95,6 +95,32 @@ def _ptr(x) -> int:
     raise TypeError(type(x))
 
 
+def _check_tensor(x, what: str, dtype_name: str, min_numel: int, device_index: Optional[int]) -> None:
+    """Shape/placement checks for a torch tensor handed to a DEVICE-pointer argument (raw integer
+    addresses are the caller's responsibility, as in C): CUDA, contiguous, the dtype the ABI reads,
+    at least the elements the call will touch, on the plan's device."""
+    if x is None or isinstance(x, int) or not hasattr(x, "data_ptr"):
+        return
+    if not getattr(x, "is_cuda", False):
+        raise ValueError(f"{what}: expected a CUDA tensor (DEVICE pointer)")
+    if not x.is_contiguous():
+        raise ValueError(f"{what}: tensor must be contiguous")
+    if str(x.dtype) != f"torch.{dtype_name}":
+        raise ValueError(f"{what}: dtype {x.dtype}, expected torch.{dtype_name}")
+    if x.numel() < min_numel:
+        raise ValueError(f"{what}: {x.numel()} elements, the call needs {min_numel}")
+    if device_index is not None and x.device.index is not None and x.device.index != device_index:
+        raise ValueError(f"{what}: on cuda:{x.device.index}, the plan lives on cuda:{device_index}")
+
+
+def _current_device() -> Optional[int]:
+    try:
+        import torch
+        return torch.cuda.current_device() if torch.cuda.is_available() else None
+    except Exception:
+        return None
+
+
 def _stream(stream) -> int:
     if stream is None:
         import torch
@@ -129,6 +155,7 @@ class Plan:
             _check(lib().epic_plan_create(ctypes.byref(self._h), grid_n, pad, self.n_ant,
                                           _ptr(uv), _ptr(taps), kernel_k), "epic_plan_create")
         self.N = lib().epic_plan_get_n(self._h)
+        self.device_index = _current_device()   # the plan's tables live on the device current at creation
         self.n_layouts = _check(lib().epic_plan_get_n_layouts(self._h), "epic_plan_get_n_layouts")
 
     # -- lifetime
@@ -198,23 +225,38 @@ class Plan:
         return tuple(int(v) for v in out)
 
     # -- device work
+    def _check_call(self, voltages, vdtype: str, per_sample: int, n_t: int, n_chan: int, n_pol: int, out_accum) -> None:
+        if n_t <= 0 or n_chan <= 0 or n_pol not in (1, 2):
+            return  # empty calls are no-ops; bad n_pol is the library's error to report
+        _check_tensor(voltages, "voltages", vdtype, n_t * n_chan * n_pol * self.n_ant * per_sample, self.device_index)
+        planes = lib().epic_plan_get_n_planes(self._h, n_pol)
+        if planes > 0:
+            _check_tensor(out_accum, "out_accum", "float32", n_chan * planes * self.N * self.N, self.device_index)
+
     def image(self, voltages, n_t: int, n_chan: int, n_pol: int, out_accum, stream=None) -> None:
         """epic_image: voltages DEVICE uint8 [T][C][Np][A]; ADDS into out_accum DEVICE float32
         [C][planes][N][N]."""
+        self._check_call(voltages, "uint8", 1, n_t, n_chan, n_pol, out_accum)
         _check(lib().epic_image(self._h, _ptr(voltages), n_t, n_chan, n_pol, _ptr(out_accum),
                                 _stream(stream)), "epic_image")
 
     def image_cf32(self, voltages, n_t: int, n_chan: int, n_pol: int, out_accum, stream=None) -> None:
         """epic_image_cf32: voltages DEVICE float32 [T][C][Np][A][2]."""
+        self._check_call(voltages, "float32", 2, n_t, n_chan, n_pol, out_accum)
         _check(lib().epic_image_cf32(self._h, _ptr(voltages), n_t, n_chan, n_pol, _ptr(out_accum),
                                      _stream(stream)), "epic_image_cf32")
 
     def autocorr_remove(self, voltages, n_t: int, n_chan: int, n_pol: int, out_accum, stream=None) -> None:
         """epic_autocorr_remove: subtract the a = b (zero-spacing) part of the same gulp."""
+        self._check_call(voltages, "uint8", 1, n_t, n_chan, n_pol, out_accum)
         _check(lib().epic_autocorr_remove(self._h, _ptr(voltages), n_t, n_chan, n_pol, _ptr(out_accum),
                                           _stream(stream)), "epic_autocorr_remove")
 
     def debug_grid(self, voltages, is_cf32: bool, n_pol: int, out_plane, stream=None, layout: int = 0) -> None:
+        if n_pol in (1, 2):
+            _check_tensor(voltages, "voltages", "float32" if is_cf32 else "uint8",
+                          n_pol * self.n_ant * (2 if is_cf32 else 1), self.device_index)
+            _check_tensor(out_plane, "out_plane", "float32", n_pol * self.N * self.N * 2, self.device_index)
         _check(lib().epic_debug_grid_layout(self._h, int(layout), _ptr(voltages), int(bool(is_cf32)), n_pol,
                                             _ptr(out_plane), _stream(stream)), "epic_debug_grid_layout")
 

@@ -19,7 +19,7 @@ SOURCES = ["epic_plan.cu", "epic_twopass.cu", "epic_fused.cu", "epic_tiled.cu", 
 HEADERS = [os.path.join(CSRC, "epic_internal.h"), os.path.join(CSRC, "epic_packed.cuh"), os.path.join(ROOT, "include", "epic.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--use_fast_math=false", "--expt-relaxed-constexpr",
+    "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr",
 ]
 
 
@@ -39,20 +39,24 @@ def _stale() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile csrc/*.cu into paper_1904_11422_b200/libepic.so; returns its path."""
+    """Compile csrc/*.cu into paper_1904_11422_b200/libepic.so; returns its path.  Objects whose
+    source and headers are older than the object are kept (force=True recompiles everything)."""
     if not force and not _stale():
         return LIB
     nvcc = _nvcc()
     objs = []
     procs = []
+    hdr_t = max(os.path.getmtime(d) for d in HEADERS + [os.path.abspath(__file__)])
     for s in SOURCES:
+        src = os.path.join(CSRC, s)
         obj = os.path.join(CSRC, s.replace(".cu", ".o"))
-        cmd = [nvcc, *[f for f in NVCC_FLAGS if f != "--use_fast_math=false"], "-I", os.path.join(ROOT, "include"),
-               "-I", CSRC, "-c", os.path.join(CSRC, s), "-o", obj]
+        objs.append(obj)
+        if not force and os.path.exists(obj) and os.path.getmtime(obj) > max(hdr_t, os.path.getmtime(src)):
+            continue
+        cmd = [nvcc, *NVCC_FLAGS, "-I", os.path.join(ROOT, "include"), "-I", CSRC, "-c", src, "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         procs.append((s, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
-        objs.append(obj)
     for s, pr in procs:
         out, _ = pr.communicate()
         if verbose or pr.returncode != 0:

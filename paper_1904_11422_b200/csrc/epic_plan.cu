@@ -446,37 +446,44 @@ int epic_plan_set_input_order(epic_plan* plan, int order) {
 
 int epic_plan_set_delay_phasors(epic_plan* plan, int n_chan, int n_pol, const float* phasors) {
   if (!plan) return EPIC_ERR_ARG;
-  EPIC_CUDA_TRY(cudaDeviceSynchronize());  // earlier calls may still read the old table
+  // validate first: a rejected call leaves the active table as it was
+  if (phasors && (n_chan < 1 || (n_pol != 1 && n_pol != 2))) return EPIC_ERR_ARG;
+  float2* d_new = nullptr;
+  float4* d_new_pair = nullptr;
+  if (phasors) {
+    const size_t A = (size_t)plan->n_ant, n = (size_t)n_chan * n_pol * A;
+    std::vector<float4> pair((size_t)n_chan * A);
+    for (int c = 0; c < n_chan; ++c)
+      for (size_t a = 0; a < A; ++a) {
+        const float* lo = phasors + (((size_t)c * n_pol + 0) * A + a) * 2;
+        const float* hi = phasors + (((size_t)c * n_pol + (n_pol - 1)) * A + a) * 2;
+        pair[(size_t)c * A + a] = make_float4(lo[0], hi[0], lo[1], hi[1]);
+      }
+    cudaError_t ce = cudaMalloc(&d_new, n * sizeof(float2));
+    if (ce == cudaSuccess) ce = cudaMalloc(&d_new_pair, pair.size() * sizeof(float4));
+    if (ce == cudaSuccess) ce = cudaMemcpy(d_new, phasors, n * sizeof(float2), cudaMemcpyHostToDevice);
+    if (ce == cudaSuccess) ce = cudaMemcpy(d_new_pair, pair.data(), pair.size() * sizeof(float4), cudaMemcpyHostToDevice);
+    if (ce != cudaSuccess) {
+      set_cuda_error(ce);
+      if (d_new) cudaFree(d_new);
+      if (d_new_pair) cudaFree(d_new_pair);
+      return ce == cudaErrorMemoryAllocation ? EPIC_ERR_NOMEM : EPIC_ERR_CUDA;
+    }
+  }
+  // swap: earlier calls may still read the old table
+  const cudaError_t se = cudaDeviceSynchronize();
+  if (se != cudaSuccess) {
+    set_cuda_error(se);
+    if (d_new) cudaFree(d_new);
+    if (d_new_pair) cudaFree(d_new_pair);
+    return EPIC_ERR_CUDA;
+  }
   if (plan->d_phasor) cudaFree(plan->d_phasor);
   if (plan->d_phasor_pair) cudaFree(plan->d_phasor_pair);
-  plan->d_phasor = nullptr;
-  plan->d_phasor_pair = nullptr;
-  plan->ph_n_chan = plan->ph_n_pol = 0;
-  if (!phasors) return EPIC_OK;
-  if (n_chan < 1 || (n_pol != 1 && n_pol != 2)) return EPIC_ERR_ARG;
-  const size_t A = (size_t)plan->n_ant, n = (size_t)n_chan * n_pol * A;
-  std::vector<float4> pair((size_t)n_chan * A);
-  for (int c = 0; c < n_chan; ++c)
-    for (size_t a = 0; a < A; ++a) {
-      const float* lo = phasors + (((size_t)c * n_pol + 0) * A + a) * 2;
-      const float* hi = phasors + (((size_t)c * n_pol + (n_pol - 1)) * A + a) * 2;
-      pair[(size_t)c * A + a] = make_float4(lo[0], hi[0], lo[1], hi[1]);
-    }
-  cudaError_t ce = cudaMalloc(&plan->d_phasor, n * sizeof(float2));
-  if (ce == cudaSuccess) ce = cudaMalloc(&plan->d_phasor_pair, pair.size() * sizeof(float4));
-  if (ce == cudaSuccess) ce = cudaMemcpy(plan->d_phasor, phasors, n * sizeof(float2), cudaMemcpyHostToDevice);
-  if (ce == cudaSuccess)
-    ce = cudaMemcpy(plan->d_phasor_pair, pair.data(), pair.size() * sizeof(float4), cudaMemcpyHostToDevice);
-  if (ce != cudaSuccess) {
-    set_cuda_error(ce);
-    if (plan->d_phasor) cudaFree(plan->d_phasor);
-    if (plan->d_phasor_pair) cudaFree(plan->d_phasor_pair);
-    plan->d_phasor = nullptr;
-    plan->d_phasor_pair = nullptr;
-    return ce == cudaErrorMemoryAllocation ? EPIC_ERR_NOMEM : EPIC_ERR_CUDA;
-  }
-  plan->ph_n_chan = n_chan;
-  plan->ph_n_pol = n_pol;
+  plan->d_phasor = d_new;
+  plan->d_phasor_pair = d_new_pair;
+  plan->ph_n_chan = phasors ? n_chan : 0;
+  plan->ph_n_pol = phasors ? n_pol : 0;
   return EPIC_OK;
 }
 

@@ -104,3 +104,14 @@ def test_bench_per_channel_variant_keeps_the_configs_shape():
     np.testing.assert_allclose(off[3], off[0] * (38e6 + 75e3) / 38e6, rtol=1e-4, atol=1e-4)
     assert bench.algorithmic_flops_per_frame(pc) == bench.algorithmic_flops_per_frame(base)
     assert pc.voltages().shape == (6, 4, 2, 256)
+
+
+def test_binding_rejects_host_tensors_for_device_pointers():
+    """binding._check_tensor: a CPU tensor, a wrong dtype or a short buffer never reaches the C ABI."""
+    import pytest
+    import torch
+    from paper_1904_11422_b200 import binding
+    with pytest.raises(ValueError):
+        binding._check_tensor(torch.zeros(16, dtype=torch.uint8), "voltages", "uint8", 16, None)
+    binding._check_tensor(1234, "voltages", "uint8", 16, None)   # raw addresses are the caller's business, as in C
+    binding._check_tensor(None, "voltages", "uint8", 16, None)

@@ -366,6 +366,58 @@ def test_autocorr_removal_leaves_only_cross_pairs_brute_force():
     assert np.allclose(got[4], got[2]) and np.allclose(got[5], -got[3])
 
 
+@pytest.mark.parametrize("n_pol,n_products", [(2, 4), (1, 1)])
+def test_autocorr_removal_multi_antenna_taps_brute_force(n_pol, n_products):
+    """Several antennas, each with its OWN random complex 3x3 taps (so every |What_a|^2 differs):
+    image minus autocorr_image equals the direct-Fourier image of the pairs a != b only, each pair
+    imaged straight from Eq. 1-2 with antenna a's tap-weighted response
+        What_a[m][l] = sum_d W_a[d] exp(+2 pi i ((cx_a+dx) l + (cy_a+dy) m) / N)
+    typed out here.  Pairing antenna a's power with another antenna's beam fails this."""
+    rng = np.random.default_rng(23 + n_pol)
+    n, n_ant, t_n, k = 16, 4, 3, 3
+    uv = rng.uniform(0, n, (n_ant, 2)).astype(np.float32)          # incl. taps that wrap past the edge
+    taps = rng.standard_normal((n_ant, k, k, 2)).astype(np.float32)
+    v = rng.standard_normal((t_n, 1, n_pol, n_ant, 2)).astype(np.float32)
+    img = orc.epic_image(v, "cf32", uv, taps, n, 1, n_products, kernel_k=k)
+    auto = orc.autocorr_image(v, "cf32", uv, taps, n, 1, n_products, kernel_k=k)
+    e = v[..., 0].astype(np.float64) + 1j * v[..., 1]                 # [T][1][Np][A]
+    w = taps[..., 0].astype(np.float64) + 1j * taps[..., 1]           # [A][dy][dx]
+    cx = np.floor(uv[:, 0].astype(np.float64) + 0.5).astype(int)
+    cy = np.floor(uv[:, 1].astype(np.float64) + 0.5).astype(int)
+    what = np.zeros((n_ant, n, n), dtype=complex)                     # [a][m][l]
+    for a in range(n_ant):
+        for m in range(n):
+            for l in range(n):
+                s = 0j
+                for iy, dy in enumerate((-1, 0, 1)):
+                    for ix, dx in enumerate((-1, 0, 1)):
+                        s += w[a, iy, ix] * np.exp(2j * np.pi * (((cx[a] + dx) * l + (cy[a] + dy) * m) % n) / n)
+                what[a, m, l] = s
+    q = n_pol - 1
+    xx = np.zeros((n, n)); yy = np.zeros((n, n)); xy = np.zeros((n, n), dtype=complex)
+    for a in range(n_ant):
+        for b in range(n_ant):
+            if a == b:
+                continue
+            fringe = what[a] * np.conj(what[b])
+            xx += ((e[:, 0, 0, a] * np.conj(e[:, 0, 0, b])).sum() * fringe).real
+            yy += ((e[:, 0, q, a] * np.conj(e[:, 0, q, b])).sum() * fringe).real
+            xy += (e[:, 0, 0, a] * np.conj(e[:, 0, q, b])).sum() * fringe
+    got = img[0] - auto[0]
+    peak = np.abs(img[0, 0]).max()
+    assert np.abs(got[0] - xx).max() <= 1e-10 * peak
+    if n_products == 4:
+        assert np.abs(got[1] - yy).max() <= 1e-10 * peak
+        assert np.abs(got[2] - xy.real).max() <= 1e-10 * peak
+        assert np.abs(got[3] - xy.imag).max() <= 1e-10 * peak
+        assert np.abs(got[4] - xy.real).max() <= 1e-10 * peak
+        assert np.abs(got[5] + xy.imag).max() <= 1e-10 * peak
+    # and the a = b part itself, antenna by antenna: sum_a V_aa |What_a|^2
+    diag = sum((np.abs(e[:, 0, 0, a]) ** 2).sum() * np.abs(what[a]) ** 2 for a in range(n_ant))
+    assert np.abs(auto[0, 0] - diag).max() <= 1e-10 * peak
+    assert np.abs(auto[0, 0] - diag[::-1, ::-1]).max() > 1e-3 * peak     # the beams are not interchangeable
+
+
 def test_autocorr_image_special_cases():
     """One antenna: the whole image is its autocorrelation.  Delta kernel: the a = b part is flat,
     sum_a sum_t |E_a|^2, whatever the cells."""
