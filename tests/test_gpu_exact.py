@@ -53,10 +53,10 @@ def _expected_flat(v, n_products):
     """v uint8 [T][C][Np][A] -> float64 [C][planes]: the flat image value of every plane."""
     e = _unpack_typed(v).sum(axis=-1)            # [T][C][Np]: all antennas share the cell
     assert np.array_equal(e, orc.unpack_ci4(v).sum(axis=-1))
-    xx = (np.abs(e[:, :, 0]) ** 2).sum(axis=0)
+    xx = (e[:, :, 0].real ** 2 + e[:, :, 0].imag ** 2).sum(axis=0)     # exact integers (np.abs would take a sqrt)
     if n_products == 1:
         return xx[:, None]
-    yy = (np.abs(e[:, :, 1]) ** 2).sum(axis=0)
+    yy = (e[:, :, 1].real ** 2 + e[:, :, 1].imag ** 2).sum(axis=0)
     if n_products == 2:
         return np.stack([xx, yy], axis=1)
     xy = (e[:, :, 0] * np.conj(e[:, :, 1])).sum(axis=0)
