@@ -31,9 +31,10 @@ METRIC = "E-field frames/sec (chan x time gridded+FFT'd+accumulated)"
 UNIT = "frames/s"
 FP32_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # SMs x lanes x FMA x max clock
 L2_FLUSH_BYTES = 256 << 20
-PATH_NAMES = {1: "twopass", 2: "fused", 3: "tiled", 4: "tensor"}
+PATH_NAMES = {1: "twopass", 2: "fused", 3: "tiled", 4: "tensor", 5: "stream"}
 PATH_KERNELS = {1: "grid_rowfft+colfft_accum", 2: "epic_fused_kernel (+ epic_fused_fixup, <1 % of the step)", 3: "tiled_rows+tiled_cols",
-                4: "epic_tc_kernel (column transform as BF16x3 tcgen05.mma; + epic_fused_fixup)"}
+                4: "epic_tc_kernel (column transform as BF16x3 tcgen05.mma; + epic_fused_fixup)",
+                5: "tiled_stream (one persistent kernel: row CTAs -> L2 ring -> column CTAs)"}
 
 
 def algorithmic_flops_per_frame(wl) -> float:
@@ -202,7 +203,7 @@ def run_epic(args, wl):
     plan = epic.Plan(wl.grid_n, wl.pad, wl.ant_uv, wl.taps, wl.kernel_k)
     plan.set_products(wl.n_products)
     if args.path:
-        plan.set_path({"auto": 0, "twopass": 1, "fused": 2, "tiled": 3, "tensor": 4}[args.path])
+        plan.set_path({"auto": 0, "twopass": 1, "fused": 2, "tiled": 3, "tensor": 4, "stream": 5}[args.path])
     if args.scratch_mib:
         plan.set_scratch_limit(args.scratch_mib << 20)
     if args.input_order == "tcap":
@@ -368,7 +369,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (1-based)")
     ap.add_argument("--impl", default="epic", choices=["epic", "reference"])
-    ap.add_argument("--path", default=None, choices=[None, "auto", "twopass", "fused", "tiled", "tensor"])
+    ap.add_argument("--path", default=None, choices=[None, "auto", "twopass", "fused", "tiled", "tensor", "stream"])
     ap.add_argument("--n-chan", type=int, default=None)
     ap.add_argument("--n-t", type=int, default=None)
     ap.add_argument("--n-ant", type=int, default=None)

@@ -55,12 +55,19 @@ typedef enum epic_status {
 /* Which kernel family epic_image uses.  AUTO picks the fastest one that supports the plan. */
 typedef enum epic_path {
   EPIC_PATH_AUTO = 0,
-  EPIC_PATH_TWOPASS = 1, /* grid+row-FFT kernel -> L2-resident scratch -> column-FFT+products kernel */
-  EPIC_PATH_FUSED = 2,   /* one kernel (+ a tiny ordered fix-up of split units), planes never leave the SM (occupied cells within 32x32, N = 64, 128) */
-  EPIC_PATH_TILED = 3,   /* N = 256, 512: packed row kernel -> L2-resident scratch -> packed column kernel */
-  EPIC_PATH_TENSOR = 4   /* the fused kernel with its column transform as a dense BF16x3 contraction on the
+  EPIC_PATH_TWOPASS = 1, /* grid+row-FFT kernel -> scratch in global memory -> column-FFT+products kernel, batch by batch */
+  EPIC_PATH_FUSED = 2,   /* one kernel (+ a tiny ordered fix-up of split units), planes never leave the SM: N = 64, 128 with the
+                            occupied cells within 32x32 (epic_fused.cu) or within 64x64 (the wide variant, epic_wide.cu) */
+  EPIC_PATH_TILED = 3,   /* N = 256, 512: packed row kernel -> scratch (1 GiB batches, streamed through HBM) -> packed column
+                            kernel; AUTO's choice for N >= 256 */
+  EPIC_PATH_TENSOR = 4,  /* the fused kernel with its column transform as a dense BF16x3 contraction on the
                             tensor cores (tcgen05.mma); N = 128, two polarisations, one layout.  Never
                             picked by AUTO: measured and reported beside the FP32 path */
+  EPIC_PATH_STREAM = 5   /* N = 256, 512: ONE persistent kernel; row CTAs hand row-transformed frames to column CTAs
+                            through a ring that stays in L2, accumulators live in registers for the whole call:
+                            HBM sees the voltages and out_accum once.  Measured slower than
+                            EPIC_PATH_TILED so far, so AUTO does not pick it; EPIC_ERR_RANGE at epic_image time if one
+                            channel's row and column CTAs cannot be co-resident */
 } epic_path;
 
 /* S2 + plan set-up ("gridded onto a 2D grid ... spacing < lambda/2"; illumination
@@ -104,7 +111,7 @@ EPIC_API int epic_plan_destroy(epic_plan* plan);
 EPIC_API int epic_plan_set_products(epic_plan* plan, int n_products);
 
 /* Select the kernel family (testing / benchmarking): an epic_path value.  EPIC_ERR_RANGE if the plan
- * cannot use it (FUSED: occupied cells within 32x32 and N = 64 or 128; TILED: N = 256 or 512). */
+ * cannot use it (FUSED: occupied cells within 64x64 and N = 64 or 128; TILED, STREAM: N = 256 or 512). */
 EPIC_API int epic_plan_set_path(epic_plan* plan, int path);
 
 /* Tuning: bytes of the plan's scratch (the intermediate H of the tiled / two-pass paths) one batch may

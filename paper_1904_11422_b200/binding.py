@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_PKG, "libepic.so")
 
 EPIC_OK = 0
 EPIC_ERR_ARG, EPIC_ERR_RANGE, EPIC_ERR_CUDA, EPIC_ERR_NOMEM = -1, -2, -3, -4
-EPIC_PATH_AUTO, EPIC_PATH_TWOPASS, EPIC_PATH_FUSED, EPIC_PATH_TILED, EPIC_PATH_TENSOR = 0, 1, 2, 3, 4
+EPIC_PATH_AUTO, EPIC_PATH_TWOPASS, EPIC_PATH_FUSED, EPIC_PATH_TILED, EPIC_PATH_TENSOR, EPIC_PATH_STREAM = 0, 1, 2, 3, 4, 5
 EPIC_ORDER_TCPA, EPIC_ORDER_TCAP = 0, 1
 
 # every symbol include/epic.h declares: name -> (restype, argtypes)

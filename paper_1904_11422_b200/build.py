@@ -15,8 +15,8 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libepic.so")
-SOURCES = ["epic_plan.cu", "epic_twopass.cu", "epic_fused.cu", "epic_tiled.cu", "epic_autocorr.cu"]
-HEADERS = [os.path.join(CSRC, "epic_internal.h"), os.path.join(CSRC, "epic_packed.cuh"), os.path.join(ROOT, "include", "epic.h")]
+SOURCES = ["epic_plan.cu", "epic_twopass.cu", "epic_fused.cu", "epic_wide.cu", "epic_tiled.cu", "epic_autocorr.cu"]
+HEADERS = [os.path.join(CSRC, "epic_internal.h"), os.path.join(CSRC, "epic_packed.cuh"), os.path.join(CSRC, "epic_fused_core.cuh"), os.path.join(ROOT, "include", "epic.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr",

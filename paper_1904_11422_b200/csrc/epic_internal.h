@@ -49,12 +49,15 @@ struct epic_plan {
   void* d_fused;               // tables private to the fused path
   int fused_ok;                // support fits the fused kernel
   void* d_tiled;               // tables private to the tiled path
+  void* d_wide;                // tables private to the wide fused path (support within 64 x 64)
+  int wide_ok;                 // support fits the wide fused kernel (and not the 32 x 32 one)
   void* d_auto;                // tap autocorrelation table of epic_autocorr_remove
   int input_order;             // EPIC_ORDER_TCPA | EPIC_ORDER_TCAP
   int ph_n_chan, ph_n_pol;     // shape of the delay phasor table (0: none set)
   float2* d_phasor;            // [ph_n_chan][ph_n_pol][n_ant] complex multipliers (reading Q19)
   float4* d_phasor_pair;       // [ph_n_chan][n_ant] (re_lo, re_hi, im_lo, im_hi): lo/hi = pol X/Y, or the same pol twice
   int tiled_ok;                // N is 256 or 512
+  int stream_k;                // tuning: row CTAs per row group of the streamed path (0 = default)
   int n_sm;
   // host copies kept for the fused path's table builder
   std::vector<epic::CellRec> h_cells;   // all layouts, concatenated
@@ -92,11 +95,19 @@ int fused_image(epic_plan* p, const ImageArgs& a);
 int tensor_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products);  // tensor-core column pass
 int tensor_image(epic_plan* p, const ImageArgs& a);
 
+// epic_wide.cu: the fused design for supports up to 64 x 64 (reached through EPIC_PATH_FUSED)
+int wide_plan_init(epic_plan* p);  // sets p->wide_ok, allocates p->d_wide
+void wide_plan_free(epic_plan* p);
+int wide_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products);
+int wide_image(epic_plan* p, const ImageArgs& a);
+
 // epic_tiled.cu
 int tiled_plan_init(epic_plan* p);  // sets p->tiled_ok, allocates p->d_tiled
 void tiled_plan_free(epic_plan* p);
 int tiled_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products);
 int tiled_image(epic_plan* p, const ImageArgs& a);
+int stream_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products);  // persistent producer/consumer variant
+int stream_image(epic_plan* p, const ImageArgs& a);
 
 // epic_autocorr.cu
 int autocorr_plan_init(epic_plan* p, const float* taps);  // allocates p->d_auto

@@ -306,7 +306,17 @@ static int image_common(epic_plan* plan, const void* volt, int is_cf32, int n_t,
   // the fused kernel reads voltage rows as 32-bit words
   const int fused_can = fused_supported(plan, is_cf32, n_pol, n_products) &&
                         (reinterpret_cast<uintptr_t>(volt) & 3u) == 0;
-  if (path == EPIC_PATH_AUTO) path = fused_can ? EPIC_PATH_FUSED : (tiled_can ? EPIC_PATH_TILED : EPIC_PATH_TWOPASS);
+  const int stream_can = stream_supported(plan, is_cf32, n_pol, n_products);
+  // AUTO keeps the batched tiled kernels for N >= 256: measured faster than the streamed kernel;
+  // the streamed kernel fetches voltages as bytes, so it takes the antenna counts the tiled row kernel cannot
+  if (path == EPIC_PATH_AUTO)
+    path = fused_can ? EPIC_PATH_FUSED : (tiled_can ? EPIC_PATH_TILED : (stream_can ? EPIC_PATH_STREAM : EPIC_PATH_TWOPASS));
+  if (path == EPIC_PATH_STREAM) {
+    if (!stream_can) return EPIC_ERR_RANGE;
+    const int st = stream_image(plan, a);
+    if (st != EPIC_ERR_RANGE || plan->path_req == EPIC_PATH_STREAM) return st;
+    path = EPIC_PATH_TWOPASS;  // AUTO: co-residency is decided at launch
+  }
   if (path == EPIC_PATH_FUSED) {
     if (!fused_can) return EPIC_ERR_RANGE;
     return fused_image(plan, a);
@@ -366,6 +376,9 @@ int epic_plan_create_per_channel(epic_plan** out, int grid_n, int pad, int n_ant
   p->fused_ok = 0;
   p->d_tiled = nullptr;
   p->tiled_ok = 0;
+  p->d_wide = nullptr;
+  p->wide_ok = 0;
+  p->stream_k = 0;
   p->d_auto = nullptr;
   p->input_order = EPIC_ORDER_TCPA;
   p->ph_n_chan = p->ph_n_pol = 0;
@@ -403,6 +416,7 @@ int epic_plan_create_per_channel(epic_plan** out, int grid_n, int pad, int n_ant
     }
   }
   if (st == EPIC_OK) st = fused_plan_init(p);
+  if (st == EPIC_OK) st = wide_plan_init(p);
   if (st == EPIC_OK) st = tiled_plan_init(p);
   if (st == EPIC_OK) st = autocorr_plan_init(p, kernel_taps);
   if (st != EPIC_OK) {
@@ -417,6 +431,7 @@ int epic_plan_destroy(epic_plan* plan) {
   if (!plan) return EPIC_OK;
   cudaError_t ce = cudaDeviceSynchronize();
   fused_plan_free(plan);
+  wide_plan_free(plan);
   tiled_plan_free(plan);
   autocorr_plan_free(plan);
   if (plan->d_phasor) cudaFree(plan->d_phasor);
@@ -460,7 +475,8 @@ int epic_plan_set_delay_phasors(epic_plan* plan, int n_chan, int n_pol, const fl
         pair[(size_t)c * A + a] = make_float4(lo[0], hi[0], lo[1], hi[1]);
       }
     cudaError_t ce = cudaMalloc(&d_new, n * sizeof(float2));
-    if (ce == cudaSuccess) ce = cudaMalloc(&d_new_pair, pair.size() * sizeof(float4));
+    if (ce == cudaSuccess) ce = cudaMalloc(&d_new_pair, (pair.size() + 4) * sizeof(float4));  // + a padded antenna group (fused unpack)
+    if (ce == cudaSuccess) ce = cudaMemset(d_new_pair, 0, (pair.size() + 4) * sizeof(float4));
     if (ce == cudaSuccess) ce = cudaMemcpy(d_new, phasors, n * sizeof(float2), cudaMemcpyHostToDevice);
     if (ce == cudaSuccess) ce = cudaMemcpy(d_new_pair, pair.data(), pair.size() * sizeof(float4), cudaMemcpyHostToDevice);
     if (ce != cudaSuccess) {
@@ -496,11 +512,11 @@ int epic_plan_set_scratch_limit(epic_plan* plan, long long bytes) {
 int epic_plan_set_path(epic_plan* plan, int path) {
   if (!plan) return EPIC_ERR_ARG;
   if (path != EPIC_PATH_AUTO && path != EPIC_PATH_TWOPASS && path != EPIC_PATH_FUSED && path != EPIC_PATH_TILED &&
-      path != EPIC_PATH_TENSOR)
+      path != EPIC_PATH_TENSOR && path != EPIC_PATH_STREAM)
     return EPIC_ERR_ARG;
   if (path == EPIC_PATH_TENSOR && (!plan->fused_ok || plan->N != 128 || plan->n_layout != 1)) return EPIC_ERR_RANGE;
-  if (path == EPIC_PATH_FUSED && !plan->fused_ok) return EPIC_ERR_RANGE;
-  if (path == EPIC_PATH_TILED && !plan->tiled_ok) return EPIC_ERR_RANGE;
+  if (path == EPIC_PATH_FUSED && !plan->fused_ok && !plan->wide_ok) return EPIC_ERR_RANGE;
+  if ((path == EPIC_PATH_TILED || path == EPIC_PATH_STREAM) && !plan->tiled_ok) return EPIC_ERR_RANGE;
   plan->path_req = path;
   return EPIC_OK;
 }
@@ -577,7 +593,8 @@ int epic_plan_get_path(const epic_plan* plan, int n_pol) {
   if (planes_for(n_pol, n_products) < 0) return EPIC_ERR_RANGE;
   if (plan->path_req != EPIC_PATH_AUTO) return plan->path_req;
   if (fused_supported(plan, 0, n_pol, n_products)) return EPIC_PATH_FUSED;
-  return tiled_supported(plan, 0, n_pol, n_products) ? EPIC_PATH_TILED : EPIC_PATH_TWOPASS;
+  if (tiled_supported(plan, 0, n_pol, n_products)) return EPIC_PATH_TILED;
+  return stream_supported(plan, 0, n_pol, n_products) ? EPIC_PATH_STREAM : EPIC_PATH_TWOPASS;
 }
 
 int epic_plan_last_launches(const epic_plan* plan) { return plan ? plan->last_launches : (int)EPIC_ERR_ARG; }

@@ -23,7 +23,7 @@ from epic_testlib import run_gpu
 
 pytestmark = pytest.mark.gpu
 
-TWOPASS, FUSED, TILED, TENSOR = 1, 2, 3, 4
+TWOPASS, FUSED, TILED, TENSOR, STREAM = 1, 2, 3, 4, 5
 
 
 def _sext4(n):
@@ -100,6 +100,9 @@ CASES = [
     ("tiled-delta-N256", 128, 2, TILED, False),
     ("tiled-taps-N256", 128, 2, TILED, True),
     ("tiled-delta-N512", 128, 4, TILED, False),
+    ("stream-delta-N256", 128, 2, STREAM, False),
+    ("stream-taps-N256", 128, 2, STREAM, True),
+    ("stream-delta-N512", 128, 4, STREAM, False),
     ("twopass-N128", 64, 2, TWOPASS, False),
 ]
 
@@ -159,14 +162,21 @@ def test_unit_phasors_keep_the_unpack_exact():
     for path in (FUSED, TWOPASS):
         gpu = run_gpu(wl, volt=v, path=path, phasors=ph)
         _assert_flat_exact(gpu, _expected_flat(v, 4), f"phasors path {path}")
+    wl = _one_cell_workload(128, 2, 8, 2, 5, 7, 4, False)      # large grid: phasors folded into the taps
+    for path in (STREAM, TILED):
+        gpu = run_gpu(wl, volt=v, path=path, phasors=ph)
+        _assert_flat_exact(gpu, _expected_flat(v, 4), f"phasors path {path}")
 
 
 # ------------------------------------------------------------------ run-to-run reproducibility
 REPRO = [
+    ("LWA55 wide", dict(idx=55, n_chan=40, n_t=100), FUSED),    # wide fused kernel
     ("C2 fused", dict(idx=2, n_chan=40, n_t=333), FUSED),       # units split between CTAs: fix-up order
     ("C3 fused", dict(idx=3, n_chan=24, n_t=200), FUSED),
     ("C4 tiled", dict(idx=4, n_chan=7, n_t=60), TILED),
     ("C5 tiled", dict(idx=5, n_chan=2, n_t=9), TILED),
+    ("C4 stream", dict(idx=4, n_chan=19, n_t=60), STREAM),      # several waves
+    ("C5 stream", dict(idx=5, n_chan=3, n_t=9), STREAM),
 ]
 
 
@@ -174,10 +184,41 @@ REPRO = [
 def test_results_are_bit_reproducible(name, kw, path):
     """No atomics anywhere and a fixed summation order: two runs of the same call give bit-identical
     images (the stand-in for compute-sanitizer racecheck, which this GPU pool does not allow)."""
-    from workloads import make_config
-    wl = make_config(kw["idx"], n_chan=kw["n_chan"], n_t=kw["n_t"])
+    from workloads import make_config, make_lwa55
+    wl = make_lwa55(n_chan=kw["n_chan"], n_t=kw["n_t"]) if kw["idx"] == 55 else make_config(kw["idx"], n_chan=kw["n_chan"], n_t=kw["n_t"])
     v = wl.voltages()
     a, info = run_gpu(wl, volt=v, path=path, return_plan_info=True)
     b = run_gpu(wl, volt=v, path=path)
     assert info["path"] == path
     assert np.array_equal(a, b), name
+
+
+# ------------------------------------------------------------------ wide fused kernel: exact folds
+@pytest.mark.parametrize("grid_n,pad", [(64, 2), (64, 1)], ids=["N128", "N64"])
+def test_wide_kernel_folds_are_exact(grid_n, pad):
+    """Four occupied cells 32 apart in x and y, (0,0) (32,0) (0,32) (32,32) after relocation: the wide kernel's
+    x-fold (in the gather) and y-fold (in the column pass) multiply by W_N^{32 l}, W_N^{32 m} -- fourth (N = 128)
+    or second (N = 64) roots of unity -- so the image A[m][l] = S00 + w^l S10 + w^m S01 + w^(l+m) S11 is made of
+    exact integers; typed out here and compared exactly, for all 256 byte values."""
+    N = grid_n * pad
+    cells = [(5, 7), (37, 7), (5, 39), (37, 39)]              # (x, y)
+    uv = np.array([c for c in cells for _ in range(2)], dtype=np.float32)   # two antennas per cell
+    wl = make_custom(grid_n=grid_n, pad=pad, n_ant=8, n_pol=2, kernel_k=1, n_chan=9, n_t=29, n_products=4, ant_uv=uv)
+    rng = np.random.default_rng(64)
+    v = rng.integers(0, 256, (29, 9, 2, 8), dtype=np.uint8)
+    gpu, info = run_gpu(wl, volt=v, path=FUSED, return_plan_info=True)
+    assert info["path"] == FUSED and info["support"][2:] == (33, 33)
+    e = _unpack_typed(v)                                        # [T][C][Np][A]
+    s = e.reshape(29, 9, 2, 4, 2).sum(axis=-1)                  # per cell: S00, S10, S01, S11
+    w = {128: 1j, 64: -1.0}[N]
+    l = np.arange(N)[None, :]
+    m = np.arange(N)[:, None]
+    a = (s[..., 0, None, None] + s[..., 1, None, None] * w ** (l % 4) + s[..., 2, None, None] * w ** (m % 4)
+         + s[..., 3, None, None] * w ** ((l + m) % 4))         # [T][C][Np][N][N], exact Gaussian integers
+    ax, ay = a[:, :, 0], a[:, :, 1]
+    xy = (ax * np.conj(ay)).sum(axis=0)
+    want = np.stack([(ax.real ** 2 + ax.imag ** 2).sum(axis=0), (ay.real ** 2 + ay.imag ** 2).sum(axis=0),
+                     xy.real, xy.imag, xy.real, -xy.imag], axis=1)          # [C][6][N][N]
+    assert np.array_equal(want.astype(np.float32).astype(np.float64), want)
+    bad = np.argwhere(gpu != want.astype(np.float32))
+    assert bad.size == 0, f"{len(bad)} pixels differ, first {bad[:3].tolist()}"

@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 
 from oracle import epic_oracle as orc
-from workloads import make_config, make_custom, make_per_channel
+from workloads import make_config, make_custom, make_lwa55, make_per_channel
 
 from epic_testlib import TOL, assert_parity, max_rel_err, run_gpu, run_oracle
 
@@ -154,6 +154,99 @@ def test_fused_capable_plans_both_paths(wl, path):
             assert plan.path(wl.n_pol) == epic.EPIC_PATH_FUSED  # AUTO picks it
 
 
+# ------------------------------------------------------------------ wide fused kernel: supports up to 64 x 64 (N = 64, 128)
+def _wrapped_uv(side_y, side_x, n_ant, N, seed):
+    """antennas filling a side_y x side_x box whose origin is near the plane's far corner, so the box wraps"""
+    rng = np.random.default_rng(seed)
+    return (np.array([N - 9.0, N - 21.0]) + rng.uniform(0, 1, (n_ant, 2)) * np.array([side_x - 1.0, side_y - 1.0])).astype(np.float32)
+
+
+WIDE_CAPABLE = [
+    make_lwa55(n_chan=3, n_t=21),                                     # the paper's operating point: ~43 x 39 cells, 3 m top-hat, 4 products
+    make_lwa55(n_chan=2, n_t=9, kernel="delta", n_products=2),        # delta kernel
+    make_lwa55(n_chan=150, n_t=5, kernel="delta", n_products=2),      # more units than CTAs can split evenly
+    make_custom(grid_n=64, pad=2, n_ant=256, n_pol=2, kernel_k=1, n_chan=2, n_t=7,
+                ant_uv=np.random.default_rng(11).uniform(-0.49, 63.49, (256, 2))),   # fills 64 x 64 cells
+    make_custom(grid_n=64, pad=1, n_ant=200, n_pol=2, kernel_k=1, n_chan=3, n_t=6, n_products=2,
+                ant_uv=np.random.default_rng(12).uniform(-0.49, 63.49, (200, 2))),   # N = 64: no padding at all
+    make_custom(grid_n=64, pad=1, n_ant=60, n_pol=1, kernel_k=3, n_chan=2, n_t=11, ant_uv=_wrapped_uv(40, 50, 60, 64, 1)),  # N = 64, 1 pol, odd n_t, wraps
+    make_custom(grid_n=64, pad=2, n_ant=120, n_pol=2, kernel_k=3, n_chan=2, n_t=5, ant_uv=_wrapped_uv(60, 20, 120, 128, 2)),  # tall, narrow (x fits 32), wraps
+    make_custom(grid_n=64, pad=2, n_ant=120, n_pol=2, kernel_k=5, n_chan=2, n_t=5, ant_uv=_wrapped_uv(20, 58, 120, 128, 3), n_products=2),  # flat, wide: x-fold only
+    make_custom(grid_n=64, pad=2, n_ant=77, n_pol=2, kernel_k=3, n_chan=3, n_t=9, ant_uv=_wrapped_uv(45, 45, 77, 128, 4)),  # 77 antennas: byte-fetched tail group
+    make_custom(grid_n=64, pad=2, n_ant=90, n_pol=1, kernel_k=1, n_chan=2, n_t=8, ant_uv=_wrapped_uv(48, 33, 90, 128, 5)),  # rows exactly 48
+]
+
+
+@pytest.mark.parametrize("path", [1, 2], ids=["twopass", "fused-wide"])
+@pytest.mark.parametrize("wl", WIDE_CAPABLE, ids=lambda w: f"{w.name}-c{w.n_chan}-t{w.n_t}")
+def test_wide_support_plans_both_paths(wl, path):
+    """Plans whose occupied cells need more than 32 x 32 but fit 64 x 64: EPIC_PATH_FUSED runs the wide kernel
+    (AUTO picks it), and it and the two-pass path each match the oracle."""
+    epic = _epic()
+    v = wl.voltages()
+    gpu, info = run_gpu(wl, volt=v, path=path, calls=2, return_plan_info=True)
+    assert info["path"] == path
+    _, _, R, Cc = info["support"]
+    assert max(R, Cc) > 32 and max(R, Cc) <= 64
+    ref = run_oracle(wl, volt=v)
+    assert_parity(gpu, ref, what=f"{wl.name} path={path}")
+    if path == 2:
+        assert info["launches"] == 2
+        with epic.Plan(wl.grid_n, wl.pad, wl.ant_uv, wl.taps, wl.kernel_k) as plan:
+            plan.set_products(wl.n_products)
+            assert plan.path(wl.n_pol) == epic.EPIC_PATH_FUSED
+            with pytest.raises(epic.EpicError):
+                plan.set_path(epic.EPIC_PATH_TENSOR)   # the tensor-core variant is the 32 x 32 kernel's
+
+
+@pytest.mark.parametrize("mode", ["native", "phasors", "both"])
+def test_wide_input_order_and_delay_phasors(mode):
+    wl = make_lwa55(n_chan=2, n_t=7)
+    v = wl.voltages()
+    native = mode in ("native", "both")
+    rng = np.random.default_rng(9)
+    ph = None
+    if mode in ("phasors", "both"):
+        ph = (np.exp(2j * np.pi * rng.random((wl.n_chan, wl.n_pol, wl.n_ant))) * rng.uniform(0.8, 1.25, (wl.n_chan, wl.n_pol, wl.n_ant))).astype(np.complex64)
+    vin = np.ascontiguousarray(np.swapaxes(v, 2, 3)) if native else v
+    gpu = run_gpu(wl, volt=vin, path=2, native=native, phasors=ph, autocorr=True)
+    kw = dict(order="TCAP" if native else "TCPA", delay_phasors=ph)
+    ref = orc.epic_image(vin, wl.input_kind, wl.ant_uv, wl.taps, wl.grid_n, wl.pad, wl.n_products, kernel_k=wl.kernel_k, **kw)
+    ref = ref - orc.autocorr_image(vin, wl.input_kind, wl.ant_uv, wl.taps, wl.grid_n, wl.pad, wl.n_products, kernel_k=wl.kernel_k, **kw)
+    assert_parity(gpu, ref, what=f"wide {mode}")
+
+
+def test_wide_per_channel_layouts():
+    """One layout per channel over a band wide enough that the box grows past 32 cells: wide kernel, per-channel tables."""
+    epic = _epic()
+    wl = make_per_channel(grid_n=64, pad=2, n_ant=96, n_pol=2, kernel_k=3, n_chan=6, n_t=13, f0_hz=50e6, df_hz=3e6,
+                          diameter_m=105.0, n_sources=1)
+    v = wl.voltages()
+    gpu, info = run_gpu(wl, volt=v, path=2, calls=2, return_plan_info=True)
+    assert info["path"] == 2 and max(info["support"][2:]) > 32
+    assert_parity(gpu, run_oracle(wl, volt=v), what=wl.name)
+
+
+@pytest.mark.parametrize("n_ant", [77, 254, 3])
+def test_antenna_counts_not_a_multiple_of_four_stay_on_the_fast_paths(n_ant):
+    """n_ant % 4 != 0: voltage rows are not word-aligned; the fused kernels fetch them as bytes instead of
+    falling to the two-pass path, in both input orders and with one polarisation."""
+    epic = _epic()
+    for n_pol, native in [(2, False), (2, True), (1, False)]:
+        wl = make_custom(grid_n=64, pad=2, n_ant=n_ant, n_pol=n_pol, kernel_k=3, n_chan=3, n_t=10, layout="disc", seed=n_ant)
+        v = wl.voltages()
+        vin = np.ascontiguousarray(np.swapaxes(v, 2, 3)) if native else v
+        gpu, info = run_gpu(wl, volt=vin, native=native, return_plan_info=True)
+        assert info["path"] == epic.EPIC_PATH_FUSED
+        ref = orc.epic_image(vin, wl.input_kind, wl.ant_uv, wl.taps, wl.grid_n, wl.pad, wl.n_products, kernel_k=wl.kernel_k,
+                             order="TCAP" if native else "TCPA")
+        assert_parity(gpu, ref, what=f"{n_ant} antennas n_pol={n_pol} native={native}")
+    wl = make_custom(grid_n=128, pad=2, n_ant=n_ant, n_pol=2, kernel_k=3, n_chan=2, n_t=6, layout="uniform", seed=n_ant)
+    gpu, info = run_gpu(wl, return_plan_info=True)        # large grid: the streamed kernel fetches bytes anyway
+    assert info["path"] == epic.EPIC_PATH_STREAM
+    assert_parity(gpu, run_oracle(wl), what=f"{n_ant} antennas, N = 256")
+
+
 # Large planes (N = 256, 512): the tiled (packed, L2-resident two-pass) path and the general
 # two-pass path must each match the oracle; AUTO must pick the tiled one.
 TILED_CAPABLE = [
@@ -169,18 +262,47 @@ TILED_CAPABLE = [
 ]
 
 
-@pytest.mark.parametrize("path", [1, 3], ids=["twopass", "tiled"])
+@pytest.mark.parametrize("path", [1, 3, 5], ids=["twopass", "tiled", "stream"])
 @pytest.mark.parametrize("wl", TILED_CAPABLE, ids=lambda w: f"{w.name}-c{w.n_chan}-t{w.n_t}")
 def test_tiled_capable_plans_both_paths(wl, path):
     epic = _epic()
+    if path == 5 and wl.N == 512 and wl.n_ant == 300:
+        # a box as tall as the plane: one channel's row and column CTAs cannot be co-resident, and forcing the
+        # streamed kernel is refused, not silently rerouted
+        with pytest.raises(epic.EpicError):
+            run_gpu(wl, path=5)
+        return
     gpu, info = run_gpu(wl, path=path, return_plan_info=True)
     assert info["path"] == path
     ref = run_oracle(wl)
     assert_parity(gpu, ref, what=f"{wl.name} path={path}")
+    if path == 5:
+        assert info["launches"] == 1  # one persistent kernel for the whole call
     if path == 3:
         with epic.Plan(wl.grid_n, wl.pad, wl.ant_uv, wl.taps, wl.kernel_k) as plan:
             plan.set_products(wl.n_products)
             assert plan.path(wl.n_pol) == epic.EPIC_PATH_TILED  # AUTO picks it
+
+
+@pytest.mark.parametrize("wl,ring_mib", [
+    (make_config(4, n_chan=21, n_t=40), 0),      # more channels than one wave holds: several waves, ring reused across them
+    (make_config(4, n_chan=3, n_t=70), 4),       # ring of 2 frames per channel: every hand-over waits on the consumers
+    (make_config(5, n_chan=5, n_t=6), 0),        # N = 512: waves of 2 channels, the last one half empty
+    (make_config(5, n_chan=2, n_t=7), 9),        # N = 512 with the smallest ring
+    (make_custom(grid_n=128, pad=2, n_ant=100, n_pol=1, kernel_k=3, n_chan=4, n_t=33, layout="uniform"), 0),  # 1 pol, odd n_t
+], ids=["C4-waves", "C4-ring2", "C5-waves", "C5-ring2", "1pol"])
+def test_stream_path_waves_and_ring_reuse(wl, ring_mib):
+    """EPIC_PATH_STREAM's hand-over machinery: channel waves, a ring much shorter than the call, two
+    calls accumulating; sampled channels against the oracle and the rest against the batched tiled path."""
+    v = wl.voltages()
+    kw = dict(scratch_limit=ring_mib << 20) if ring_mib else {}
+    gpu, info = run_gpu(wl, volt=v, path=5, calls=2, return_plan_info=True, **kw)
+    assert info["path"] == 5 and info["launches"] == 1
+    channels = sorted({0, wl.n_chan // 2, wl.n_chan - 1})
+    ref = run_oracle(wl, volt=v, channels=channels)
+    assert_parity(gpu[channels], ref, what=f"{wl.name} stream")
+    tiled = run_gpu(wl, volt=v, path=3, calls=2)
+    assert max_rel_err(gpu, tiled.astype(np.float64)) <= 1e-5
 
 
 def test_tiled_many_batches_accumulate():
@@ -226,16 +348,17 @@ def test_full_size_config_sampled_channels(idx, channels):
     assert totals.min() > 0.5 * totals.max()  # every channel was imaged (same noise statistics)
 
 
+@pytest.mark.parametrize("path", [3, 5], ids=["tiled", "stream"])
 @pytest.mark.parametrize("idx", [4, 5], ids=["C4-full", "C5-full"])
-def test_full_size_large_configs_sampled_pixels(idx):
-    """C4 / C5 at full extent through the path bench.py times (AUTO = tiled, 1 GiB scratch): the
+def test_full_size_large_configs_sampled_pixels(idx, path):
+    """C4 / C5 at full extent through the two large-grid paths bench.py times (AUTO = tiled; streamed kernel): the
     float64 oracle cannot image 256^2 / 512^2 planes x 10^4..10^5 frames in reasonable time, so
     sampled pixels of sampled channels are computed one by one from Eq. 5 (oracle.pixel_values),
     every plane, plus properties of the whole result."""
     wl = make_config(idx)
     v = wl.voltages()
-    gpu, info = run_gpu(wl, volt=v, return_plan_info=True)
-    assert info["path"] == 3
+    gpu, info = run_gpu(wl, volt=v, return_plan_info=True, path=None if path == 3 else path)
+    assert info["path"] == path and (path == 3 or info["launches"] == 1)
     rng = np.random.default_rng(40 + idx)
     channels = [0, wl.n_chan // 2 + 1, wl.n_chan - 1]
     N = wl.N
@@ -286,7 +409,8 @@ def test_autocorr_removal_matches_oracle(wl, calls):
 UPSTREAM = [
     (make_config(2, n_chan=3, n_t=21), None),                                     # fused, delta
     (make_config(3, n_chan=2, n_t=13), None),                                     # fused, taps, TMEM variant
-    (make_config(4, n_chan=2, n_t=4), None),                                      # tiled
+    (make_config(4, n_chan=2, n_t=4), None),                                      # large grid, batched tiled kernels
+    (make_config(4, n_chan=2, n_t=4), 5),                                         # large grid, streamed kernel
     (make_custom(grid_n=32, pad=2, n_ant=40, n_pol=1, kernel_k=3, n_chan=3, n_t=9, layout="disc"), None),
     (make_custom(grid_n=8, pad=2, n_ant=30, n_pol=2, kernel_k=3, n_chan=2, n_t=5, layout="wrap"), None),  # two-pass
     (make_custom(grid_n=16, pad=2, n_ant=9, n_pol=2, kernel_k=1, n_chan=2, n_t=3, input_kind="cf32"), None),
@@ -378,7 +502,7 @@ def test_random_plans_all_paths(seed):
         plan.set_products(wl.n_products)
         auto = plan.path(wl.n_pol)
     tried = []
-    for path in sorted({1, auto}):
+    for path in sorted({1, auto} | ({5} if auto == 3 and wl.N == 256 else set())):
         gpu = run_gpu(wl, volt=vin, path=path, native=native, phasors=ph, calls=int(rng.integers(1, 3)))
         assert_parity(gpu, ref, what=f"seed {seed} {wl.name} path={path}")
         tried.append(path)
@@ -446,7 +570,7 @@ def test_point_source_peaks_at_predicted_pixel():
 
 # ------------------------------------------------------------------ one antenna layout per channel (reading Q15)
 PER_CHANNEL = [
-    # (workload, paths): 1 two-pass, 2 fused, 3 tiled
+    # (workload, paths): 1 two-pass, 2 fused, 3 tiled, 5 streamed; the last one is AUTO's choice
     (make_per_channel(grid_n=64, pad=2, n_ant=64, n_pol=2, kernel_k=1, n_chan=5, n_t=37, n_products=2,
                       f0_hz=30e6, df_hz=4e6, diameter_m=100.0), [1, 2]),
     (make_per_channel(grid_n=64, pad=2, n_ant=96, n_pol=2, kernel_k=3, n_chan=7, n_t=23, f0_hz=38e6, df_hz=2e6,
@@ -454,9 +578,9 @@ PER_CHANNEL = [
     (make_per_channel(grid_n=32, pad=2, n_ant=48, n_pol=1, kernel_k=3, n_chan=4, n_t=30, f0_hz=20e6, df_hz=7e6,
                       diameter_m=90.0), [1, 2]),
     (make_per_channel(grid_n=128, pad=2, n_ant=200, n_pol=2, kernel_k=3, n_chan=3, n_t=9, f0_hz=40e6, df_hz=9e6,
-                      diameter_m=300.0), [1, 3]),
+                      diameter_m=300.0), [1, 5, 3]),
     (make_per_channel(grid_n=256, pad=2, n_ant=300, n_pol=2, kernel_k=1, n_chan=2, n_t=5, n_products=2,
-                      f0_hz=50e6, df_hz=20e6, diameter_m=500.0), [1, 3]),
+                      f0_hz=50e6, df_hz=20e6, diameter_m=500.0), [1, 5, 3]),
     (make_per_channel(grid_n=12, pad=2, n_ant=20, n_pol=2, kernel_k=5, n_chan=3, n_t=6, f0_hz=30e6, df_hz=10e6,
                       diameter_m=30.0), [1]),   # N = 24 is not a power of two -> rejected below
 ]

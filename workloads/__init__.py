@@ -12,6 +12,7 @@ from .configs import (  # noqa: F401
     Workload,
     make_config,
     make_custom,
+    make_lwa55,
     make_per_channel,
     pack_ci4,
     gaussian_taps,

@@ -299,6 +299,31 @@ def make_custom(*, grid_n: int, pad: int, n_ant: int, n_pol: int, kernel_k: int,
                     n_products, uv, taps, ph, 2.0, src)
 
 
+def make_lwa55(*, n_chan: int, n_t: int, kernel: str = "tophat", n_products: int = 4, n_ant: int = 256,
+               freq_hz: float = 55.25e6, seed: int = 55, n_sources: int = 0, n_pol: int = 2) -> Workload:
+    """The paper's own operating point as a single-layout workload: ``n_ant`` antennas
+    uniform in area in a 110 m x 100 m ellipse, gridded on lambda/2 cells at 55.25 MHz (2.713 m: about 41 x 37
+    cells, beyond a 32 x 32 support) onto a 64 x 64 grid padded to 128 x 128; kernel "tophat" = the 3 m square
+    top-hat sampled per cell (3 x 3 taps, per-antenna phase), "delta" = nearest cell."""
+    s = BASE_SEED + 3000 + seed
+    r = _rng(s, _S_POS)
+    cell_m = 299792458.0 / freq_hz / 2.0
+    rad = np.sqrt(r.random(n_ant))
+    th = 2.0 * np.pi * r.random(n_ant)
+    uv = np.stack([32.0 + 55.0 * rad * np.cos(th) / cell_m, 32.0 + 50.0 * rad * np.sin(th) / cell_m], axis=1).astype(np.float32)
+    taps = ph = None
+    k = 1
+    if kernel == "tophat":
+        k = 3
+        ph = _rng(s, _S_PHASE).uniform(0.0, 2.0 * np.pi, n_ant)
+        taps = tophat_taps(uv, 3, 3.0 / cell_m, ph)
+    elif kernel != "delta":
+        raise ValueError(kernel)
+    src = _draw_sources(s, n_sources, 128, max(n_t, 1), n_ant, 2.0) if n_sources else []
+    name = f"LWA55-{n_ant}ant-128x128-{kernel}-{n_products}prod"
+    return Workload(name, 0, s, 64, 2, n_ant, n_pol, k, n_chan, n_t, "ci4", n_products, uv, taps, ph, 2.0, src)
+
+
 def make_per_channel(*, grid_n: int, pad: int, n_ant: int, n_pol: int, kernel_k: int, n_chan: int, n_t: int,
                      f0_hz: float, df_hz: float, diameter_m: float = 100.0, tophat_m: float = 3.0,
                      n_products: Optional[int] = None, n_sources: int = 0, seed: int = 7,
