@@ -25,7 +25,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from workloads import make_config, make_per_channel  # noqa: E402
+from workloads import make_config, make_custom, make_lwa55, make_per_channel  # noqa: E402
 
 METRIC = "E-field frames/sec (chan x time gridded+FFT'd+accumulated)"
 UNIT = "frames/s"
@@ -69,6 +69,20 @@ def per_channel_variant(wl):
     pc.name = f"{wl.name}+per-channel-cells"
     pc.index = wl.index
     return pc
+
+
+def make_wide_workload(kind: str, n_chan: int, n_t: int):
+    """Workloads whose occupied cells need more than 32 x 32 (the wide fused kernel), C2's extent."""
+    if kind == "lwa55-tophat":
+        wl = make_lwa55(n_chan=n_chan, n_t=n_t, kernel="tophat", n_products=4)
+    elif kind == "lwa55-delta":
+        wl = make_lwa55(n_chan=n_chan, n_t=n_t, kernel="delta", n_products=2)
+    else:
+        uv = np.random.default_rng(64).uniform(-0.49, 63.49, (256, 2)).astype(np.float32)
+        wl = make_custom(grid_n=64, pad=2, n_ant=256, n_pol=2, kernel_k=1, n_chan=n_chan, n_t=n_t, n_products=2, ant_uv=uv)
+        wl.name = "fill64-256ant-128x128-delta-XXYY"
+    wl.index = 2
+    return wl
 
 
 def max_over_ranks(values, device) -> list:
@@ -133,6 +147,140 @@ class ClockSampler:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
         return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
                 "samples": len(sm), "reasons": sorted(reasons)}
+
+
+HBM_FALLBACK_GBS = 6650.0  # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+def measured_hbm_gbs():
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except (OSError, ValueError, KeyError):
+        return HBM_FALLBACK_GBS, "B200_PROFILING.md fallback"
+
+
+def measured_traffic(wl_name: str, path: int):
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of this workload and kernel family
+    from the ncu captures summarised in profiles/traffic.csv, or None."""
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        with open(tpath) as fh:
+            rows = dict(ln.strip().split(",")[:2] for ln in fh.read().splitlines()[1:] if "," in ln)
+        key = f"{wl_name}:{PATH_NAMES.get(path)}"
+        return int(rows[key]) if key in rows else None
+    except (OSError, ValueError):
+        return None
+
+
+def roofline_of(wl, kernel_ms: float, path: int, probe_tflops=None) -> dict:
+    """BASELINE.json north_star: the roofline is the SLOWER of (FFT + gridding + product flops at FP32 peak) and
+    (voltage + image bytes at HBM bandwidth); both sides are computed and `bound` says which one binds."""
+    flops = algorithmic_flops_per_frame(wl)
+    bytes_f = algorithmic_bytes_per_frame(wl)
+    hbm_gbs, hbm_kind = measured_hbm_gbs()
+    t_alu = flops * wl.frames / (FP32_NOMINAL_TFLOPS * 1e12)
+    t_hbm = bytes_f * wl.frames / (hbm_gbs * 1e9)
+    achieved = flops * wl.frames / (kernel_ms * 1e-3) / 1e12
+    r = {
+        "bound": "alu" if t_alu >= t_hbm else "hbm", "achieved": achieved, "peak": FP32_NOMINAL_TFLOPS, "unit": "TFLOP/s",
+        "frac": max(t_alu, t_hbm) / (kernel_ms * 1e-3), "traffic": measured_traffic(wl.name, path),
+        "frac_kind": "algorithmic work (SURVEY.md 8(d)) / measured time; the kernels execute less than the algorithmic count where they prune",
+        "peak_kind": "nominal FP32: 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
+        "t_alu_ms": t_alu * 1e3, "t_hbm_ms": t_hbm * 1e3, "hbm_peak_gbs": hbm_gbs, "hbm_peak_kind": hbm_kind,
+        "algorithmic_flops_per_frame": flops, "algorithmic_bytes_per_frame": bytes_f,
+        "algorithmic_bytes_per_launch": bytes_f * wl.frames,
+        "hbm_achieved_gbs": bytes_f * wl.frames / (kernel_ms * 1e-3) / 1e9,
+        "kernel_ms": kernel_ms, "kernel": PATH_KERNELS.get(path, str(path)),
+    }
+    if probe_tflops:
+        r["peak_measured_fma_probe"] = probe_tflops
+        r["frac_of_measured_probe"] = achieved / probe_tflops
+    return r
+
+
+def time_other_config(label: str, wl, dev, steps: int, warmup: int, path=None, probe_tflops=None) -> dict:
+    """Device-resident timing of another workload in the same process (same rules: L2 flushed between
+    iterations, CUDA events on the launching stream); returns a compact record for `other_configs`."""
+    import torch
+    import paper_1904_11422_b200 as epic
+    t0 = time.perf_counter()
+    volt = wl.voltages()
+    d_volt = torch.from_numpy(volt).to(dev)
+    plan = epic.Plan(wl.grid_n, wl.pad, wl.ant_uv, wl.taps, wl.kernel_k)
+    try:
+        plan.set_products(wl.n_products)
+        if path is not None:
+            plan.set_path(path)
+        out = torch.zeros((wl.n_chan, plan.n_planes(wl.n_pol), wl.N, wl.N), dtype=torch.float32, device=dev)
+        flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+        stream = torch.cuda.current_stream()
+        ms = []
+        for i in range(warmup + steps):
+            out.zero_()
+            flush.fill_(1)
+            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            plan.image(d_volt, wl.n_t, wl.n_chan, wl.n_pol, out, stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            if i >= warmup:
+                ms.append(e0.elapsed_time(e1))
+        used = plan.path(wl.n_pol)
+        launches = plan.last_launches()
+        support = plan.support()
+    finally:
+        plan.destroy()
+    mean_ms = float(np.mean(ms))
+    roof = roofline_of(wl, mean_ms, used, probe_tflops)
+    return {"label": label, "workload": wl.name, "kernel_path": PATH_NAMES.get(used, str(used)), "value": wl.frames / (mean_ms * 1e-3),
+            "unit": UNIT, "ms_per_step": mean_ms, "ms_per_step_median": float(np.median(ms)), "ms_per_step_min": float(np.min(ms)),
+            "steps": steps, "warmup": warmup, "launches_per_step": launches, "support_box": list(support),
+            "frac": roof["frac"], "frac_of_measured_probe": roof.get("frac_of_measured_probe"), "bound": roof["bound"],
+            "traffic": roof["traffic"], "algorithmic_bytes_per_launch": roof["algorithmic_bytes_per_launch"],
+            "setup_s": round(time.perf_counter() - t0, 1)}
+
+
+def _cpu_worker(job):
+    """One channel of the bounded sample in a worker process (all-cores leg of cpu_baseline)."""
+    os.environ.setdefault("OMP_NUM_THREADS", "1")
+    from oracle import epic_oracle as orc
+    (volt_c, kind, ant_uv, taps, grid_n, pad, n_products, kernel_k, order) = job
+    orc.epic_image(volt_c, kind, ant_uv, taps, grid_n, pad, n_products, kernel_k=kernel_k, mode="fast", order=order)
+    return volt_c.shape[0]
+
+
+def cpu_baseline_all_cores(wl, volt, order: str = "TCPA", seconds_hint: float = 10.0, single_fps: float = 1.0) -> dict:
+    """the same oracle fanned over os.cpu_count() processes, one channel each (channels are
+    independent); the time-sample count per channel is cut so that the leg stays near `seconds_hint`."""
+    import multiprocessing as mp
+    n_proc = os.cpu_count() or 1
+    n_jobs = min(wl.n_chan, n_proc)
+    n_t = int(max(1, min(volt.shape[0], single_fps * seconds_hint)))   # every process images n_t frames
+    jobs = []
+    for c in range(n_jobs):
+        uv = wl.ant_uv[c] if wl.ant_uv.ndim == 3 else wl.ant_uv
+        tp = None if wl.taps is None else (wl.taps[c] if wl.ant_uv.ndim == 3 else wl.taps)
+        vc = np.ascontiguousarray(volt[:n_t, c:c + 1])
+        jobs.append((vc, wl.input_kind, uv, tp, wl.grid_n, wl.pad, wl.n_products, wl.kernel_k, order))
+    ctx = mp.get_context("fork")
+    t0 = time.perf_counter()
+    with ctx.Pool(n_jobs) as pool:
+        done = pool.map(_cpu_worker, jobs)
+    dt = time.perf_counter() - t0
+    frames = int(sum(done))
+    return {"value": frames / dt, "unit": UNIT, "cores": n_jobs, "kind": "oracle",
+            "sample": f"{n_jobs} processes x 1 channel x {n_t} time samples of {wl.name} ({frames} frames, {dt:.1f} s, numpy float64, "
+                      f"one thread per process, pool start-up included)"}
+
+
+def cpu_model() -> str:
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.startswith("model name"):
+                return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
 def cpu_baseline(wl, volt, n_chan_sample: int, order: str = "TCPA") -> dict:
@@ -279,13 +427,14 @@ def run_epic(args, wl):
     dev_ms = [a.elapsed_time(b) for a, b in evs]
     total_ms = float(sum(dev_ms))
 
-    for _ in range(2):
-        step_e2e()
+    run_e2e = step_device if args.no_e2e else step_e2e   # --no-e2e (profiling runs): the e2e object then repeats the device leg
+    for _ in range(0 if args.no_e2e else 2):
+        run_e2e()
     barrier()
-    evs = [step_e2e() for _ in range(args.steps)]
+    evs = [run_e2e() for _ in range(1 if args.no_e2e else args.steps)]
     barrier()
     clocks = sampler.stop() if rank == 0 else None  # sampled over both timed regions
-    e2e_ms = float(sum(a.elapsed_time(b) for a, b in evs))
+    e2e_ms = float(sum(a.elapsed_time(b) for a, b in evs)) * (args.steps if args.no_e2e else 1)
 
     total_ms, e2e_ms = max_over_ranks([total_ms, e2e_ms], dev)
     path = plan.path(wl.n_pol)
@@ -301,23 +450,12 @@ def run_epic(args, wl):
     ms_per_step = total_ms / args.steps
     value = frames_step / (ms_per_step * 1e-3)
     e2e_value = frames_step / (e2e_ms / args.steps * 1e-3)
-    flops = algorithmic_flops_per_frame(wl)
-    bytes_f = algorithmic_bytes_per_frame(wl)
     kernel_ms = float(np.mean(dev_ms))           # rank 0's own kernel time (one launch per step when fused)
-    achieved = flops * wl.frames / (kernel_ms * 1e-3) / 1e12
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.csv")   # measured DRAM bytes per launch (profiles/traffic.md)
-    if os.path.exists(tpath):
-        try:
-            with open(tpath) as fh:
-                rows = dict(ln.strip().split(",")[:2] for ln in fh.read().splitlines()[1:] if "," in ln)
-            key = f"{wl.name}:{PATH_NAMES.get(path)}"
-            traffic = int(rows[key]) if key in rows else None
-        except (OSError, ValueError):
-            traffic = None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step,
+        "ms_per_step_median": float(np.median(dev_ms)), "ms_per_step_min": float(np.min(dev_ms)),
+        "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": wl.name, **{k: v for k, v in wl.describe().items() if k != "workload"},
                    "kernel_path": PATH_NAMES.get(path, str(path)),
@@ -325,18 +463,12 @@ def run_epic(args, wl):
                    "layouts": int(wl.ant_uv.shape[0]) if wl.ant_uv.ndim == 3 else 1,
                    "support_box": list(support), "l2": f"flushed between iterations ({L2_FLUSH_BYTES >> 20} MiB write)",
                    "sharding": "independent replicas of the workload per GPU (channels are independent), no collective"},
-        "roofline": {
-            "bound": "alu", "achieved": achieved, "peak": FP32_NOMINAL_TFLOPS, "unit": "TFLOP/s",
-            "frac": achieved / FP32_NOMINAL_TFLOPS, "traffic": traffic,
-            "peak_kind": "nominal FP32: 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
-            "peak_measured_fma_probe": probe["tflops"], "frac_of_measured_probe": achieved / probe["tflops"],
-            "algorithmic_flops_per_frame": flops, "algorithmic_bytes_per_frame": bytes_f,
-            "hbm_achieved_gbs": bytes_f * wl.frames / (kernel_ms * 1e-3) / 1e9,
-            "kernel_ms": kernel_ms, "kernel": PATH_KERNELS.get(path, str(path)),
-        },
+        "roofline": roofline_of(wl, kernel_ms, path, probe["tflops"]),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(volt.nbytes),
-                "d2h_bytes_per_step": int(out.numel() * 4),
-                "how": f"{n_chunks} time chunks (the first half as long as the others), H2D of chunk k+1 overlapped with epic_image of chunk k, one D2H of out_accum"},
+                "d2h_bytes_per_step": int(out.numel() * 4), "measured": not args.no_e2e,
+                "how": f"the C ABI takes DEVICE pointers (include/epic.h), so the host legs are torch copy_() on pinned memory "
+                       f"around it: {n_chunks} time chunks (the first half as long as the others), H2D of chunk k+1 on a copy "
+                       f"stream overlapped with epic_image of chunk k, one D2H of out_accum; all inside the timed region"},
         "gpu_launches": int(launches),
         "clocks": clocks,
     }
@@ -353,10 +485,38 @@ def run_epic(args, wl):
         line["roofline"]["tensor"] = {"executed_bf16_tflops": exe, "peak": bf16_peak, "frac": exe / bf16_peak,
                                       "peak_kind": kind, "executed_mma_flops_per_frame": per_frame,
                                       "note": "BF16 hi/lo split: 3 products per real product, 4 real per complex"}
+    if world == 1 and args.other_configs and wl.index == 2 and not args.workload and not args.per_channel_cells \
+            and args.n_chan is None and args.n_t is None:
+        # the other BASELINE.json configurations and the variants DESIGN.md reports, device-resident, fewer steps
+        # (C5 is 33 ms per step); the clocks line above does not cover them, so each run is bracketed by its own sample
+        import paper_1904_11422_b200 as epic_mod
+        others = [("C3", make_config(3), None), ("C4", make_config(4), None), ("C5", make_config(5), None),
+                  ("C4 streamed kernel", make_config(4), epic_mod.EPIC_PATH_STREAM),
+                  ("C5 streamed kernel", make_config(5), epic_mod.EPIC_PATH_STREAM),
+                  ("C2 tensor-core column pass", make_config(2), epic_mod.EPIC_PATH_TENSOR),
+                  ("LWA 55.25 MHz, 3 m top-hat, 4 products (wide fused kernel)", make_wide_workload("lwa55-tophat", 128, 1000), None),
+                  ("LWA 55.25 MHz, delta, XX YY (wide fused kernel)", make_wide_workload("lwa55-delta", 128, 1000), None)]
+        sampler2 = ClockSampler(local)
+        sampler2.start()
+        recs = []
+        for label, w2, pth in others:
+            try:
+                recs.append(time_other_config(label, w2, dev, steps=5, warmup=3, path=pth, probe_tflops=probe["tflops"]))
+            except Exception as exc:  # a failed extra must not cost the headline line
+                recs.append({"label": label, "error": repr(exc)})
+        line["other_configs"] = {"records": recs, "clocks": sampler2.stop(),
+                                 "note": "device-resident inputs, 3 warm-up + 5 timed steps each, L2 flushed between iterations"}
     if world == 1 and not args.no_cpu_baseline:
         # bounded sample: the oracle's cost per frame grows with the plane (N^2 log N), so fewer channels of the big configs
         n_cpu = max(1, args.cpu_channels * (128 * 128) // max(128 * 128, wl.N * wl.N * wl.n_planes // 2))
-        line["cpu_baseline"] = cpu_baseline(wl, volt, n_cpu, args.input_order.upper())
+        cb = cpu_baseline(wl, volt, n_cpu, args.input_order.upper())
+        cb["cpu_model"] = cpu_model()
+        cb["host_cores"] = os.cpu_count()
+        try:
+            cb["all_cores"] = cpu_baseline_all_cores(wl, volt, args.input_order.upper(), 8.0, cb["value"])
+        except Exception as exc:
+            cb["all_cores"] = {"error": repr(exc)}
+        line["cpu_baseline"] = cb
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -375,6 +535,9 @@ def main():
     ap.add_argument("--n-ant", type=int, default=None)
     ap.add_argument("--cpu-channels", type=int, default=16, help="channels of the workload the oracle images for cpu_baseline (~13 s on C2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="profiling runs only: skip the host-buffer leg (its object is then not a measurement)")
+    ap.add_argument("--no-other-configs", dest="other_configs", action="store_false",
+                    help="skip the other_configs block (C3, C4, C5, streamed, tensor, wide) of the default C2 run")
     ap.add_argument("--input-order", default="tcpa", choices=["tcpa", "tcap"], help="tcap = [T][C][A][Np], transposed in the load")
     ap.add_argument("--delay-phasors", action="store_true", help="apply per-(channel, pol, antenna) delay phasors")
     ap.add_argument("--e2e-chunks", type=int, default=4, help="time chunks of the end-to-end leg (H2D overlapped)")
@@ -382,8 +545,15 @@ def main():
     ap.add_argument("--per-channel-cells", action="store_true",
                     help="configs 2-4 with one antenna layout per 25 kHz channel (cell = lambda_c/2) and, for 3 and 4, "
                          "the 3 m top-hat kernel (PAPER.md:122, 162-168)")
+    ap.add_argument("--workload", default=None, choices=[None, "lwa55-tophat", "lwa55-delta", "fill64"],
+                    help="instead of --config: the paper's operating point (256 antennas, 110 m x 100 m, lambda/2 cells at "
+                         "55.25 MHz, PAPER.md:148, 166-168) with the 3 m top-hat / four products or the delta kernel / XX, YY; "
+                         "or 256 antennas uniformly filling all 64 x 64 cells (delta, XX, YY)")
     args = ap.parse_args()
-    wl = make_config(args.config, n_chan=args.n_chan, n_t=args.n_t, n_ant=args.n_ant)
+    if args.workload:
+        wl = make_wide_workload(args.workload, args.n_chan or 128, args.n_t or 1000)
+    else:
+        wl = make_config(args.config, n_chan=args.n_chan, n_t=args.n_t, n_ant=args.n_ant)
     if args.per_channel_cells:
         wl = per_channel_variant(wl)
     if args.impl == "reference":
