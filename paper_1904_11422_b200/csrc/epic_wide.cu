@@ -14,7 +14,7 @@
 // it is applied in the GATHER: a cell (y, x >= 32) is summed into the folded cell (y, x - 32) times
 // W_Q^{l2}.  The shared plane stays 32 cells wide ([rows][34] float4) and the row pass is the
 // 32 x 32 kernel's, unchanged.  Along y the column pass folds the up-to-four row blocks while loading.
-// Two pairs per batch (a plane is up to 64 x 34 x 16 B = 34.8 KB) keep two CTAs on an SM.
+// Two to four pairs per batch, by plane height (a plane is up to 64 x 34 x 16 B = 34.8 KB), keep two CTAs on an SM.
 #include <algorithm>
 #include <cmath>
 #include <cstring>
@@ -28,7 +28,6 @@
 namespace epic {
 namespace {
 
-constexpr int FW = 2;  // pairs per batch
 
 // column fold: z[bitrev(y)] = in[y] + c32 in[y+32] + c16 (in[y+16] + c32 in[y+48]); rows y+32 exist while
 // y < NB2, rows y+48 while y < NB3 (RA = 32: neither, 48: NB2 = 16, 64: both)
@@ -110,7 +109,7 @@ __device__ __forceinline__ void col_task_wide_tmem(const float4* __restrict__ co
 // S3 with the x-fold: every thread owns cell slots tid + j NT of the R x 32 folded block (sorted by entry
 // count); a slot's list holds first the entries of cell (y, x), then those of cell (y, x + 32), whose sum
 // enters times fx = W_Q^{l2}.  Sums in table order, no atomics.
-template <int NT, int PLW>
+template <int NT, int PLW, int FW>
 __device__ __forceinline__ void gather_wide(const FusedParams& P, const float4* __restrict__ E, float4* __restrict__ gh,
                                             const uint2* __restrict__ info, int n_slot, float fxr, float fxi) {
   for (int s = threadIdx.x; s < n_slot; s += NT) {
@@ -149,8 +148,8 @@ __device__ __forceinline__ void gather_wide(const FusedParams& P, const float4* 
   }
 }
 
-// RA: rows allocated per plane (32, 48 or 64 >= R; rows R .. RA-1 stay zero)
-template <int Q, int NPROD, int RA>
+// RA: rows allocated per plane (32, 48 or 64 >= R; rows R .. RA-1 stay zero); FW: pairs per batch
+template <int Q, int NPROD, int RA, int FW>
 __global__ void __launch_bounds__(64 * Q, 2) epic_wide_kernel(FusedParams P) {
   constexpr int NT = 64 * Q, N = 32 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1), PLW = RA * HS;
   constexpr int NB2 = RA > 32 ? 16 : 0, NB3 = RA > 48 ? 16 : 0;
@@ -261,7 +260,7 @@ __global__ void __launch_bounds__(64 * Q, 2) epic_wide_kernel(FusedParams P) {
     // x-fold constant of the unit: W_Q^{l2} (Q = 4: i^l2, Q = 2: (-1)^l2), exact
     const float fxr = Q == 4 ? (float)((l2 == 0) - (l2 == 2)) : (float)(1 - 2 * l2);
     const float fxi = Q == 4 ? (float)((l2 == 1) - (l2 == 3)) : 0.0f;
-    gather_wide<NT, PLW>(P, E, gh, info, n_slot, fxr, fxi);
+    gather_wide<NT, PLW, FW>(P, E, gh, info, n_slot, fxr, fxi);
     __syncthreads();
 
     for (int base = warp * 32; base < ntask; base += NT) {
@@ -305,15 +304,16 @@ struct WideTables {
 };
 
 template <int Q>
-size_t wide_smem_bytes(int ra, int n_ant_pad, int R) {
+size_t wide_smem_bytes(int ra, int fw, int n_ant_pad, int R) {
+  const size_t FW = (size_t)fw;
   return ((size_t)FW * ra * HS + (size_t)2 * Q * TWV + (size_t)FW * n_ant_pad) * sizeof(float4) + (size_t)R * S * sizeof(uint2);
 }
 
-template <int Q, int NPROD, int RA>
+template <int Q, int NPROD, int RA, int FW>
 int launch_wide(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
   constexpr int NT = 64 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
-  const size_t smem = wide_smem_bytes<Q>(RA, P.n_ant, P.R);
-  auto kern = epic_wide_kernel<Q, NPROD, RA>;
+  const size_t smem = wide_smem_bytes<Q>(RA, FW, P.n_ant, P.R);
+  auto kern = epic_wide_kernel<Q, NPROD, RA, FW>;
   if (smem > 48 * 1024)
     EPIC_CUDA_TRY(cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int per_sm = 0;
@@ -330,17 +330,29 @@ int launch_wide(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
 }
 
 template <int Q, int NPROD>
-int launch_wide_ra(const epic_plan* p, const FusedParams& P, int ra, cudaStream_t s) {
-  if (ra == 32) return launch_wide<Q, NPROD, 32>(p, P, s);
-  if (ra == 48) return launch_wide<Q, NPROD, 48>(p, P, s);
-  return launch_wide<Q, NPROD, 64>(p, P, s);
+int launch_wide_ra(const epic_plan* p, const FusedParams& P, int ra, int fw, cudaStream_t s) {
+  if (ra == 32) return launch_wide<Q, NPROD, 32, 4>(p, P, s);
+  if (ra == 48) return fw == 3 ? launch_wide<Q, NPROD, 48, 3>(p, P, s) : launch_wide<Q, NPROD, 48, 2>(p, P, s);
+  return launch_wide<Q, NPROD, 64, 2>(p, P, s);
 }
 
 template <int Q>
-int launch_wide_q(const epic_plan* p, const FusedParams& P, int n_products, int ra, cudaStream_t s) {
-  if (n_products == 1) return launch_wide_ra<Q, 1>(p, P, ra, s);
-  if (n_products == 2) return launch_wide_ra<Q, 2>(p, P, ra, s);
-  return launch_wide_ra<Q, 4>(p, P, ra, s);
+int launch_wide_q(const epic_plan* p, const FusedParams& P, int n_products, int ra, int fw, cudaStream_t s) {
+  if (n_products == 1) return launch_wide_ra<Q, 1>(p, P, ra, fw, s);
+  if (n_products == 2) return launch_wide_ra<Q, 2>(p, P, ra, fw, s);
+  return launch_wide_ra<Q, 4>(p, P, ra, fw, s);
+}
+
+// pairs per batch: as many as keep two CTAs on an SM, and for 48-row planes the count (2 or 3) that leaves
+// fewer idle lanes in the row pass (FW * R * 2 tasks on rounds of 64 Q threads)
+int wide_fw(int Q, int ra, int R, int n_ant_pad) {
+  if (ra == 32) return 4;
+  if (ra == 64) return 2;
+  const int nt = 64 * Q;
+  auto eff = [&](int fw) { const int tasks = fw * R * 2; return (double)tasks / (double)(((tasks + nt - 1) / nt) * nt); };
+  const size_t smem3 = Q == 2 ? wide_smem_bytes<2>(ra, 3, n_ant_pad, R) : wide_smem_bytes<4>(ra, 3, n_ant_pad, R);
+  if (2 * (smem3 + 1024) > (size_t)227 * 1024) return 2;
+  return eff(3) >= eff(2) ? 3 : 2;
 }
 
 }  // namespace
@@ -452,8 +464,9 @@ int wide_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products) {
   if (!((n_pol == 1 && n_products == 1) || (n_pol == 2 && (n_products == 2 || n_products == 4)))) return 0;
   const WideTables* wt = static_cast<const WideTables*>(p->d_wide);
   const int Q = p->N / S, nt = 64 * Q, a_pad = (p->n_ant + 3) & ~3;
-  if ((long long)FW * (a_pad / 4) > (long long)MAXW * nt) return 0;  // prefetch registers
-  const size_t smem = Q == 2 ? wide_smem_bytes<2>(wt->ra, a_pad, p->R) : wide_smem_bytes<4>(wt->ra, a_pad, p->R);
+  const int fw = wide_fw(Q, wt->ra, p->R, a_pad);
+  if ((long long)fw * (a_pad / 4) > (long long)MAXW * nt) return 0;  // prefetch registers
+  const size_t smem = Q == 2 ? wide_smem_bytes<2>(wt->ra, fw, a_pad, p->R) : wide_smem_bytes<4>(wt->ra, fw, a_pad, p->R);
   return smem <= (size_t)200 * 1024 ? 1 : 0;
 }
 
@@ -481,10 +494,11 @@ int wide_image(epic_plan* p, const ImageArgs& a) {
   P.n_planes = a.n_planes;
   P.R = p->R;
   P.Cc = p->Cc;
-  const int per_batch = a.n_pol == 2 ? FW : 2 * FW;  // time samples per batch
+  const int fw = wide_fw(Q, wt->ra, p->R, P.n_ant);
+  const int per_batch = a.n_pol == 2 ? fw : 2 * fw;  // time samples per batch
   P.nb = (a.n_t + per_batch - 1) / per_batch;
   P.total = (long long)a.n_chan * Q * P.nb;
-  const int st = Q == 2 ? launch_wide_q<2>(p, P, a.n_products, wt->ra, a.stream) : launch_wide_q<4>(p, P, a.n_products, wt->ra, a.stream);
+  const int st = Q == 2 ? launch_wide_q<2>(p, P, a.n_products, wt->ra, fw, a.stream) : launch_wide_q<4>(p, P, a.n_products, wt->ra, fw, a.stream);
   if (st != EPIC_OK) return st;
   p->last_launches = 2;  // the wide kernel and the (tiny) fix-up of split units
   return EPIC_OK;
