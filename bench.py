@@ -240,6 +240,37 @@ def time_other_config(label: str, wl, dev, steps: int, warmup: int, path=None, p
             "setup_s": round(time.perf_counter() - t0, 1)}
 
 
+def run_sweep(args):
+    """Paper-figure analogues, one JSON line per point, device-resident inputs:
+    --sweep grid: image side N in {32, 64, 128, 256} with the SAME 256 dual-pol antennas (C2's disc layout scaled
+                  to the same fraction of the aperture grid), delta kernel, XX and YY, 128 channels x 1000 samples
+                  (PAPER.md:204, 249 Fig. 8: run time against grid size);
+    --sweep gulp: C2 with n_t samples per epic_image call in {50, ..., 2500} (Fig. 7: gulp size)."""
+    import torch
+    import paper_1904_11422_b200 as epic
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    probe = epic.epic_fp32_peak_probe(20000)
+    points = []
+    if args.sweep == "grid":
+        base = make_config(2, n_chan=1, n_t=1)
+        for grid_n in (16, 32, 64, 128):
+            uv = (grid_n / 2.0 + (base.ant_uv.astype(np.float64) - 32.0) * (grid_n / 64.0)).astype(np.float32)
+            wl = make_custom(grid_n=grid_n, pad=2, n_ant=256, n_pol=2, kernel_k=1, n_chan=128, n_t=1000, n_products=2, ant_uv=uv)
+            wl.name = f"sweep-grid-256ant-{2 * grid_n}x{2 * grid_n}-delta-XXYY"
+            points.append((f"N = {2 * grid_n}", wl))
+    else:
+        for n_t in (50, 125, 250, 500, 1000, 2500):
+            points.append((f"n_t = {n_t} per call", make_config(2, n_t=n_t)))
+    for label, wl in points:
+        rec = time_other_config(label, wl, dev, steps=args.steps, warmup=max(args.warmup, 3), probe_tflops=probe["tflops"])
+        rec.update({"sweep": args.sweep, "metric": METRIC, "n_chan": wl.n_chan, "n_t": wl.n_t, "N": wl.N, "n_ant": wl.n_ant,
+                    "flops_per_frame": algorithmic_flops_per_frame(wl)})
+        print(json.dumps(rec))
+
+
 def _cpu_worker(job):
     """One channel of the bounded sample in a worker process (all-cores leg of cpu_baseline)."""
     os.environ.setdefault("OMP_NUM_THREADS", "1")
@@ -549,7 +580,12 @@ def main():
                     help="instead of --config: the paper's operating point (256 antennas, 110 m x 100 m, lambda/2 cells at "
                          "55.25 MHz, PAPER.md:148, 166-168) with the 3 m top-hat / four products or the delta kernel / XX, YY; "
                          "or 256 antennas uniformly filling all 64 x 64 cells (delta, XX, YY)")
+    ap.add_argument("--sweep", default=None, choices=[None, "grid", "gulp"],
+                    help="paper-figure analogues: image side at fixed antennas (Fig. 8) or samples per call (Fig. 7); one JSON line per point")
     args = ap.parse_args()
+    if args.sweep:
+        run_sweep(args)
+        return
     if args.workload:
         wl = make_wide_workload(args.workload, args.n_chan or 128, args.n_t or 1000)
     else:

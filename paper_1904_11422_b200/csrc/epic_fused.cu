@@ -57,15 +57,16 @@ namespace {
 // STG: the gather's (antenna, tap) tables are copied to shared memory once per CTA (tap kernels of
 // one-layout plans whose tables fit beside two resident CTAs): their reads leave the L1/L2 path,
 // C3 +2.8 % (measured); the delta kernels, whose table is 2 bytes per antenna, gain nothing.
-template <int Q, int NPROD, bool DELTA, int NB, bool PC, bool STG>
+// FF: pairs per batch
+template <int Q, int NPROD, bool DELTA, int NB, bool PC, bool STG, int FF = F>
 __global__ void __launch_bounds__(64 * Q, 2)
 epic_fused_kernel(FusedParams P) {
   static_assert(!(STG && (DELTA || PC)), "staged tables: tap kernels of one-layout plans only");
   constexpr int NT = 64 * Q, N = 32 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  float4* gh = reinterpret_cast<float4*>(smem_raw);  // [F][32][HS]
-  float4* tws = gh + F * PLANE;                      // [2Q][TWV]
-  float4* E = tws + 2 * Q * TWV;                     // [F][A]
+  float4* gh = reinterpret_cast<float4*>(smem_raw);  // [FF][32][HS]
+  float4* tws = gh + FF * PLANE;                      // [2Q][TWV]
+  float4* E = tws + 2 * Q * TWV;                     // [FF][A]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
   // static, contiguous share of the (unit-major, batch-minor) work list
@@ -80,9 +81,9 @@ epic_fused_kernel(FusedParams P) {
 #pragma unroll
   for (int j = 0; j < S * S / NT; ++j)
     info[j] = __ldg(P.cell_info + (PC ? (size_t)(unit / Q) * (S * S) : (size_t)0) + tid + j * NT);
-  for (int i = tid; i < F * PLANE; i += NT) gh[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);  // rows >= R stay zero
+  for (int i = tid; i < FF * PLANE; i += NT) gh[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);  // rows >= R stay zero
   for (int i = tid; i < 2 * Q * TWV; i += NT) tws[i] = __ldg(P.tw + i);
-  float2* tap_s = reinterpret_cast<float2*>(E + F * P.n_ant);       // [n_ent] (STG only)
+  float2* tap_s = reinterpret_cast<float2*>(E + FF * P.n_ant);       // [n_ent] (STG only)
   uint16_t* ant_s = reinterpret_cast<uint16_t*>(tap_s + P.n_ent);   // [n_ent]
   if constexpr (STG) {
     for (int i = tid; i < P.n_ent; i += NT) { tap_s[i] = __ldg(P.ent_tap + i); ant_s[i] = __ldg(P.ent_ant + i); }
@@ -166,20 +167,20 @@ epic_fused_kernel(FusedParams P) {
   const int first_unit = unit;
   int seg_begin = b;  // first batch of the current unit done by this CTA
   PrefetchSlots ps;
-  prefetch_init<NT>(P, tid, ps);
+  prefetch_init<NT, FF>(P, tid, ps);
   uint32_t wlo[MAXW], whi[MAXW];
-  prefetch_batch<NT>(P, ps, unit / Q, b, wlo, whi);
+  prefetch_batch<NT, FF>(P, ps, unit / Q, b, wlo, whi);
   unpack_batch<DELTA>(P, ps, E, wlo, whi, unit / Q);
   __syncthreads();
 
-  const int ntask = F * P.R * 2;
+  const int ntask = FF * P.R * 2;
   for (long long g = g0; g < g1; ++g) {
     int unit_n = unit, b_n = b + 1;
     if (b_n == P.nb) { b_n = 0; ++unit_n; }
     const bool more = g + 1 < g1;
-    if (more) prefetch_batch<NT>(P, ps, unit_n / Q, b_n, wlo, whi);
+    if (more) prefetch_batch<NT, FF>(P, ps, unit_n / Q, b_n, wlo, whi);
 
-    gather_batch<NT, DELTA, STG, DELTA>(P, E, gh, info, ant_s, tap_s);
+    gather_batch<NT, DELTA, STG, DELTA, FF>(P, E, gh, info, ant_s, tap_s);
     __syncthreads();
 
     const int l2 = unit % Q;
@@ -195,7 +196,7 @@ epic_fused_kernel(FusedParams P) {
 
     if (more) unpack_batch<DELTA>(P, ps, E, wlo, whi, unit_n / Q);  // E was last read by this batch's gather
 #pragma unroll 1
-    for (int f = 0; f < F; ++f) {
+    for (int f = 0; f < FF; ++f) {
       // launder the table offset: the twiddles are re-read per task, not held in 18 registers
       int tw_off = rho * TWV;
       asm volatile("" : "+r"(tw_off));
@@ -486,17 +487,17 @@ struct FusedTables {
 };
 
 template <int Q>
-size_t fused_smem_bytes(int n_ant) {
-  return ((size_t)F * PLANE + (size_t)2 * Q * TWV + (size_t)F * n_ant) * sizeof(float4);
+size_t fused_smem_bytes(int n_ant, int ff = F) {
+  return ((size_t)ff * PLANE + (size_t)2 * Q * TWV + (size_t)ff * n_ant) * sizeof(float4);
 }
 
 inline size_t fused_stage_bytes(int n_ent) { return ((size_t)n_ent * (sizeof(float2) + sizeof(uint16_t)) + 15) & ~(size_t)15; }
 
-template <int Q, int NPROD, bool DELTA, int NB, bool PC, bool STG = false>
+template <int Q, int NPROD, bool DELTA, int NB, bool PC, bool STG = false, int FF = F>
 int launch_fused(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
   constexpr int NT = 64 * Q;
-  const size_t smem = fused_smem_bytes<Q>(P.n_ant) + (STG ? fused_stage_bytes(P.n_ent) : 0);
-  auto kern = epic_fused_kernel<Q, NPROD, DELTA, NB, PC, STG>;
+  const size_t smem = fused_smem_bytes<Q>(P.n_ant, FF) + (STG ? fused_stage_bytes(P.n_ent) : 0);
+  auto kern = epic_fused_kernel<Q, NPROD, DELTA, NB, PC, STG, FF>;
   if (smem > 48 * 1024)
     EPIC_CUDA_TRY(cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int per_sm = 0;
@@ -735,7 +736,10 @@ static void fill_params(const epic_plan* p, const ImageArgs& a, FusedParams& P) 
   P.n_planes = a.n_planes;
   P.R = p->R;
   P.Cc = p->Cc;
-  const int per_batch = a.n_pol == 2 ? F : 2 * F;  // time samples per batch
+  // measured on C2 (R = 25): 5 pairs per batch fill the row pass's 256 lanes (250 instead of 200 tasks) but change
+  // nothing (31.3 M against 31.5 M frames/s) -- the SM's other CTA already covers the idle warp; 4 stays
+  P.pairs_per_batch = F;
+  const int per_batch = a.n_pol == 2 ? P.pairs_per_batch : 2 * P.pairs_per_batch;  // time samples per batch
   P.nb = (a.n_t + per_batch - 1) / per_batch;
   P.total = (long long)a.n_chan * Q * P.nb;
 }

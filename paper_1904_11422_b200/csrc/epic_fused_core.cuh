@@ -69,6 +69,7 @@ struct FusedParams {
   int unaligned;             // n_ant_true % 4 != 0: voltage rows are not word-aligned, the tail group is short
   int n_ent;                 // gather entries (one layout)
   int R, Cc;                 // occupied rows / columns of the block
+  int pairs_per_batch;       // pairs per batch the launch was sized for (epic_fused_kernel's FF)
   int nb;                    // batches per unit
   long long total;           // n_chan * Q * nb batches in all
 };
@@ -166,7 +167,7 @@ __device__ __forceinline__ void unpack_batch(const FusedParams& P, const Prefetc
 // EB (delta kernel, at most 16 antennas per cell, no delay phasors): the four values of an antenna
 // are bytes 0..15 of one word, so a cell's sum is ONE integer add per antenna and pair -- the byte
 // sums stay below 256 -- turned into floats once per cell: exact, like the float adds it replaces.
-template <int NT, bool DELTA, bool STG = false, bool EB = false>
+template <int NT, bool DELTA, bool STG = false, bool EB = false, int FF = F>
 __device__ __forceinline__ void gather_batch(const FusedParams& P, const float4* __restrict__ E,
                                              float4* __restrict__ gh, const uint2 (&info)[S * S / NT],
                                              const uint16_t* __restrict__ ant_s = nullptr,
@@ -177,32 +178,32 @@ __device__ __forceinline__ void gather_batch(const FusedParams& P, const float4*
     const uint32_t beg = info[j].x >> 8, cnt = info[j].x & 0xFFu;
     if constexpr (EB) {
       const uint32_t* Eb = reinterpret_cast<const uint32_t*>(E);
-      uint32_t sum[F];
+      uint32_t sum[FF];
 #pragma unroll
-      for (int f = 0; f < F; ++f) sum[f] = 0u;
+      for (int f = 0; f < FF; ++f) sum[f] = 0u;
       for (uint32_t e = beg; e < beg + cnt; ++e) {
         const uint32_t* ea = Eb + __ldg(P.ent_ant + e);
 #pragma unroll
-        for (int f = 0; f < F; ++f) sum[f] += ea[f * P.n_ant];
+        for (int f = 0; f < FF; ++f) sum[f] += ea[f * P.n_ant];
       }
       const float2 bias = f2(-(12582912.0f + 8.0f * (float)cnt));  // mantissa trick of epic_packed.cuh, cnt biases of 8
       float4* dst = gh + info[j].y;
 #pragma unroll
-      for (int f = 0; f < F; ++f) {
+      for (int f = 0; f < FF; ++f) {
         const float2 vr = __fadd2_rn(make_float2(biased_byte_to_float_bits(sum[f], 0), biased_byte_to_float_bits(sum[f], 1)), bias);
         const float2 vi = __fadd2_rn(make_float2(biased_byte_to_float_bits(sum[f], 2), biased_byte_to_float_bits(sum[f], 3)), bias);
         dst[f * PLANE] = make_float4(vr.x, vr.y, vi.x, vi.y);
       }
       continue;
     }
-    float2 sr[F], si[F];
+    float2 sr[FF], si[FF];
 #pragma unroll
-    for (int f = 0; f < F; ++f) { sr[f] = make_float2(0.0f, 0.0f); si[f] = make_float2(0.0f, 0.0f); }
+    for (int f = 0; f < FF; ++f) { sr[f] = make_float2(0.0f, 0.0f); si[f] = make_float2(0.0f, 0.0f); }
     for (uint32_t e = beg; e < beg + cnt; ++e) {
       const float4* ea = E + (STG ? (uint32_t)ant_s[e] : (uint32_t)__ldg(P.ent_ant + e));
       if (DELTA) {
 #pragma unroll
-        for (int f = 0; f < F; ++f) {
+        for (int f = 0; f < FF; ++f) {
           const float4 v = ea[f * P.n_ant];
           sr[f] = __fadd2_rn(sr[f], make_float2(v.x, v.y));
           si[f] = __fadd2_rn(si[f], make_float2(v.z, v.w));
@@ -211,7 +212,7 @@ __device__ __forceinline__ void gather_batch(const FusedParams& P, const float4*
         const float2 w = STG ? tap_s[e] : __ldg(P.ent_tap + e);
         const float2 wr = f2(w.x), wi = f2(w.y);
 #pragma unroll
-        for (int f = 0; f < F; ++f) {
+        for (int f = 0; f < FF; ++f) {
           const float4 v = ea[f * P.n_ant];
           const float2 vr = make_float2(v.x, v.y), vi = make_float2(v.z, v.w);
           sr[f] = __ffma2_rn(vr, wr, sr[f]); sr[f] = __ffma2_rn(neg2(vi), wi, sr[f]);
@@ -221,7 +222,7 @@ __device__ __forceinline__ void gather_batch(const FusedParams& P, const float4*
     }
     float4* dst = gh + info[j].y;
 #pragma unroll
-    for (int f = 0; f < F; ++f) dst[f * PLANE] = make_float4(sr[f].x, sr[f].y, si[f].x, si[f].y);
+    for (int f = 0; f < FF; ++f) dst[f * PLANE] = make_float4(sr[f].x, sr[f].y, si[f].x, si[f].y);
   }
 }
 

@@ -496,6 +496,7 @@ int wide_image(epic_plan* p, const ImageArgs& a) {
   P.Cc = p->Cc;
   const int fw = wide_fw(Q, wt->ra, p->R, P.n_ant);
   const int per_batch = a.n_pol == 2 ? fw : 2 * fw;  // time samples per batch
+  P.pairs_per_batch = fw;
   P.nb = (a.n_t + per_batch - 1) / per_batch;
   P.total = (long long)a.n_chan * Q * P.nb;
   const int st = Q == 2 ? launch_wide_q<2>(p, P, a.n_products, wt->ra, fw, a.stream) : launch_wide_q<4>(p, P, a.n_products, wt->ra, fw, a.stream);
