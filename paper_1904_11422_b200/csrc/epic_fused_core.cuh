@@ -93,37 +93,43 @@ __device__ __forceinline__ void prefetch_init(const FusedParams& P, int tid, Pre
 
 // global -> registers: the voltages of batch b of channel c (F pairs x A antennas).  Time samples
 // past n_t read as the zero sample.
+// Antenna counts that are no multiple of 4: voltage rows are not word-aligned, so the four samples of a slot
+// (antennas a0 .. a0+3 of time samples t_lo / t_hi of channel c) are fetched as bytes; antennas past the end read
+// as the zero sample.  Returns (word of the lo plane, word of the hi plane) as prefetch_batch makes them.
+__device__ __noinline__ uint2 fetch_slot_bytes(const uint8_t* __restrict__ volt, int n_t, int n_chan, int n_ant, int n_pol,
+                                               int native, int c, int t_lo, int t_hi, int a0) {
+  const size_t row_bytes = (size_t)n_pol * n_ant;
+  uint32_t wlo = 0u, whi = 0u;
+  for (int i = 0; i < 4; ++i) {
+    if (a0 + i >= n_ant) break;
+    if (native && n_pol == 2) {
+      if (t_lo < n_t) {
+        const uint8_t* src = volt + ((size_t)t_lo * n_chan + c) * row_bytes + 2 * (a0 + i);
+        wlo |= (uint32_t)__ldg(src) << (8 * i);
+        whi |= (uint32_t)__ldg(src + 1) << (8 * i);
+      }
+    } else {
+      const uint8_t* base = volt + (size_t)c * row_bytes + a0 + i;
+      if (t_lo < n_t) wlo |= (uint32_t)__ldg(base + (size_t)t_lo * n_chan * row_bytes) << (8 * i);
+      if (t_hi < n_t) whi |= (uint32_t)__ldg(base + (size_t)t_hi * n_chan * row_bytes + (n_pol == 2 ? n_ant : 0)) << (8 * i);
+    }
+  }
+  return make_uint2(wlo, whi);
+}
+
 template <int NT, int FF = F>
 __device__ __forceinline__ void prefetch_batch(const FusedParams& P, const PrefetchSlots& ps, int c, int b,
                                                uint32_t (&wlo)[MAXW], uint32_t (&whi)[MAXW]) {
   const int tmul = P.n_pol == 2 ? 1 : 2, thi = P.n_pol == 2 ? 0 : 1, hi_off = P.n_pol == 2 ? P.n_ant_true : 0;
   const size_t row_bytes = (size_t)P.n_pol * P.n_ant_true;
-  // antenna counts that are no multiple of 4: rows are not word-aligned, so the four samples of a slot are
-  // fetched as bytes (the antennas past the end read as the zero sample)
-  auto bytes4 = [&](const uint8_t* src, int a0, int stride) {
-    uint32_t w = 0u;
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-      if (a0 + i < P.n_ant_true) w |= (uint32_t)__ldg(src + i * stride) << (8 * i);
-    return w;
-  };
 #pragma unroll
   for (int k = 0; k < MAXW; ++k) {
     wlo[k] = 0u; whi[k] = 0u;
     if (ps.j[k] >= 0) {
       const int t_lo = (b * FF + ps.j[k]) * tmul, t_hi = t_lo + thi;
-      if (P.unaligned) {
-        if (P.native && P.n_pol == 2) {
-          if (t_lo < P.n_t) {
-            const uint8_t* src = P.volt + ((size_t)t_lo * P.n_chan + c) * row_bytes + 2 * ps.a[k];
-            wlo[k] = bytes4(src, ps.a[k], 2);
-            whi[k] = bytes4(src + 1, ps.a[k], 2);
-          }
-        } else {
-          const uint8_t* base = P.volt + (size_t)c * row_bytes + ps.a[k];
-          if (t_lo < P.n_t) wlo[k] = bytes4(base + (size_t)t_lo * P.n_chan * row_bytes, ps.a[k], 1);
-          if (t_hi < P.n_t) whi[k] = bytes4(base + (size_t)t_hi * P.n_chan * row_bytes + hi_off, ps.a[k], 1);
-        }
+      if (P.unaligned) {  // rare path, kept out of line: inlined it cost the 128-register kernels 88 bytes of spills
+        const uint2 w = fetch_slot_bytes(P.volt, P.n_t, P.n_chan, P.n_ant_true, P.n_pol, P.native, c, t_lo, t_hi, ps.a[k]);
+        wlo[k] = w.x; whi[k] = w.y;
         continue;
       }
       if (P.native && P.n_pol == 2) {  // (a X, a Y) byte pairs: two words hold this slot's four antennas
