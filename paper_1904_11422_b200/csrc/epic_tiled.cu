@@ -496,7 +496,9 @@ __device__ __forceinline__ void stream_rows_role(const StreamParams& S, float4* 
       }
     }
     // S1 input: the bytes of this group's entries for one pair (PAPER.md:120 input orders)
-    uint32_t pf[PF_MAX];
+    // The two bytes of an entry stay in separate registers until put(): combining them at the load would make every
+    // load wait for its data there (measured: 15 % of the row role's stall samples were this one line; C5 +32 %)
+    uint32_t pf[PF_MAX], pg[PF_MAX];
     auto fetch = [&](int pair) {
       const int t_lo = P.n_pol == 2 ? pair : 2 * pair, t_hi = P.n_pol == 2 ? pair : 2 * pair + 1;
       const uint8_t* lo = P.volt + ((size_t)t_lo * P.n_chan + c) * row_bytes;
@@ -505,14 +507,14 @@ __device__ __forceinline__ void stream_rows_role(const StreamParams& S, float4* 
 #pragma unroll
       for (int k = 0; k < PF_MAX; ++k) {
         const int e = tid + k * NT_S;
-        pf[k] = 0u;
+        pf[k] = 0u; pg[k] = 0u;
         if (e < n_e) {
           const uint32_t a = ant[e];
           if (P.native && P.n_pol == 2) {
             pf[k] = __ldg(reinterpret_cast<const uint16_t*>(lo + 2 * a));  // (a X, a Y) adjacent bytes
           } else {
             pf[k] = __ldg(lo + a);
-            if (have_hi) pf[k] |= (uint32_t)__ldg(hi + a) << 8;
+            if (have_hi) pg[k] = __ldg(hi + a);
           }
         }
       }
@@ -521,7 +523,7 @@ __device__ __forceinline__ void stream_rows_role(const StreamParams& S, float4* 
 #pragma unroll
       for (int k = 0; k < PF_MAX; ++k) {
         const int e = tid + k * NT_S;
-        if (e < n_e) stage[b * cap + e] = (uint16_t)pf[k];
+        if (e < n_e) stage[b * cap + e] = (uint16_t)(pf[k] | (pg[k] << 8));
       }
     };
     __syncthreads();  // ant[] and crec[] are complete
