@@ -131,6 +131,17 @@ EPIC_API int epic_plan_set_scratch_limit(epic_plan* plan, long long bytes);
 EPIC_API int epic_image(epic_plan* plan, const void* voltages, int n_t, int n_chan, int n_pol,
                float* out_accum, epic_stream stream);
 
+/* The same gulp from HOST memory, end to end: voltages_host HOST uint8 (layout as in epic_image; pinned memory makes the
+ * copies asynchronous, pageable memory works), out_accum_host HOST float[n_chan][planes][N][N].  The library cuts the gulp
+ * into n_chunks time chunks (<= 0: 4; the first one half as long, its copy is the one nothing hides), copies chunk k+1
+ * host->device on its own stream while epic_image of chunk k runs (double-buffered device staging owned by the plan),
+ * and copies the accumulated images back.  accumulate != 0: the images are ADDED to the contents of out_accum_host (which
+ * is copied to the device first); accumulate == 0: out_accum_host is overwritten.  SYNCHRONOUS: returns when
+ * out_accum_host is complete.  Honours products, path, input order, delay phasors and per-channel layouts like epic_image.
+ * This is the call bench.py's `e2e` leg times. */
+EPIC_API int epic_image_host(epic_plan* plan, const void* voltages_host, int n_t, int n_chan, int n_pol,
+                    float* out_accum_host, int accumulate, int n_chunks);
+
 /* Same with complex fp32 voltages: DEVICE float[n_t][n_chan][n_pol][n_ant][2] (re, im). */
 EPIC_API int epic_image_cf32(epic_plan* plan, const void* voltages_cf32, int n_t, int n_chan, int n_pol,
                     float* out_accum, epic_stream stream);

@@ -32,6 +32,7 @@ SYMBOLS = {
     "epic_plan_set_delay_phasors": (_i, [_vp, _i, _i, _vp]),
     "epic_image": (_i, [_vp, _vp, _i, _i, _i, _vp, _vp]),
     "epic_image_cf32": (_i, [_vp, _vp, _i, _i, _i, _vp, _vp]),
+    "epic_image_host": (_i, [_vp, _vp, _i, _i, _i, _vp, _i, _i]),
     "epic_autocorr_remove": (_i, [_vp, _vp, _i, _i, _i, _vp, _vp]),
     "epic_plan_get_n": (_i, [_vp]),
     "epic_plan_get_n_planes": (_i, [_vp, _i]),
@@ -240,6 +241,24 @@ class Plan:
         _check(lib().epic_image(self._h, _ptr(voltages), n_t, n_chan, n_pol, _ptr(out_accum),
                                 _stream(stream)), "epic_image")
 
+    def image_host(self, voltages_host, n_t: int, n_chan: int, n_pol: int, out_accum_host, accumulate: bool = True,
+                   n_chunks: int = 0) -> None:
+        """epic_image_host: the same gulp from HOST memory (numpy arrays or CPU torch tensors, pinned or not): the
+        library pipelines the host->device copies with the kernels and copies the images back; synchronous."""
+        for x, what, dt, need in ((voltages_host, "voltages_host", "uint8", n_t * n_chan * n_pol * self.n_ant),
+                                  (out_accum_host, "out_accum_host", "float32",
+                                   n_chan * max(lib().epic_plan_get_n_planes(self._h, n_pol), 0) * self.N * self.N)):
+            if isinstance(x, np.ndarray):
+                if x.dtype != np.dtype(dt) or not x.flags["C_CONTIGUOUS"] or x.size < need:
+                    raise ValueError(f"{what}: need a C-contiguous {dt} array of at least {need} elements")
+            elif hasattr(x, "data_ptr"):
+                if getattr(x, "is_cuda", False) or not x.is_contiguous() or str(x.dtype) != f"torch.{dt}" or x.numel() < need:
+                    raise ValueError(f"{what}: need a contiguous CPU {dt} tensor of at least {need} elements")
+            elif x is not None and not isinstance(x, int):
+                raise TypeError(type(x))
+        _check(lib().epic_image_host(self._h, _ptr(voltages_host), n_t, n_chan, n_pol, _ptr(out_accum_host),
+                                     int(bool(accumulate)), int(n_chunks)), "epic_image_host")
+
     def image_cf32(self, voltages, n_t: int, n_chan: int, n_pol: int, out_accum, stream=None) -> None:
         """epic_image_cf32: voltages DEVICE float32 [T][C][Np][A][2]."""
         self._check_call(voltages, "float32", 2, n_t, n_chan, n_pol, out_accum)
@@ -279,6 +298,10 @@ def epic_plan_destroy(plan: Optional[Plan]) -> None:
 
 def epic_image(plan: Plan, voltages, n_t, n_chan, n_pol, out_accum, stream=None) -> None:
     plan.image(voltages, n_t, n_chan, n_pol, out_accum, stream)
+
+
+def epic_image_host(plan: Plan, voltages_host, n_t, n_chan, n_pol, out_accum_host, accumulate=True, n_chunks=0) -> None:
+    plan.image_host(voltages_host, n_t, n_chan, n_pol, out_accum_host, accumulate, n_chunks)
 
 
 def epic_image_cf32(plan: Plan, voltages, n_t, n_chan, n_pol, out_accum, stream=None) -> None:

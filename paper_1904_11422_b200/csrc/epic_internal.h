@@ -33,6 +33,18 @@ struct DevTables {
 
 } // namespace epic
 
+namespace epic {
+// epic_image_host: double-buffered device staging of the voltages, a device copy of out_accum, two streams
+struct HostPipe {
+  cudaStream_t compute, copy;
+  cudaEvent_t copied[2], consumed[2];
+  void* d_volt[2];
+  size_t volt_bytes;   // capacity of each staging buffer
+  float* d_out;
+  size_t out_bytes;    // capacity of d_out
+};
+}  // namespace epic
+
 struct epic_plan {
   int grid_n, pad, N, logN, n_ant, K;
   int n_products_req; // 0 = default
@@ -58,6 +70,7 @@ struct epic_plan {
   float4* d_phasor_pair;       // [ph_n_chan][n_ant] (re_lo, re_hi, im_lo, im_hi): lo/hi = pol X/Y, or the same pol twice
   int tiled_ok;                // N is 256 or 512
   int stream_k;                // tuning: row CTAs per row group of the streamed path (0 = default)
+  epic::HostPipe* pipe;        // streams, events and device staging of epic_image_host (created on first use)
   int n_sm;
   // host copies kept for the fused path's table builder
   std::vector<epic::CellRec> h_cells;   // all layouts, concatenated

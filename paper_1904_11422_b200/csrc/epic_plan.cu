@@ -332,6 +332,61 @@ static int image_common(epic_plan* plan, const void* volt, int is_cf32, int n_t,
   return twopass_image(plan, a);
 }
 
+static void host_pipe_free(epic_plan* plan) {
+  HostPipe* hp = plan->pipe;
+  if (!hp) return;
+  for (int i = 0; i < 2; ++i) {
+    if (hp->d_volt[i]) cudaFree(hp->d_volt[i]);
+    if (hp->copied[i]) cudaEventDestroy(hp->copied[i]);
+    if (hp->consumed[i]) cudaEventDestroy(hp->consumed[i]);
+  }
+  if (hp->d_out) cudaFree(hp->d_out);
+  if (hp->compute) cudaStreamDestroy(hp->compute);
+  if (hp->copy) cudaStreamDestroy(hp->copy);
+  delete hp;
+  plan->pipe = nullptr;
+}
+
+// streams and events on first use; device buffers grown on demand
+static int host_pipe_prepare(epic_plan* plan, size_t chunk_bytes, size_t out_bytes) {
+  if (!plan->pipe) {
+    HostPipe* hp = new (std::nothrow) HostPipe();
+    if (!hp) return EPIC_ERR_NOMEM;
+    std::memset(hp, 0, sizeof(*hp));
+    plan->pipe = hp;
+    EPIC_CUDA_TRY(cudaStreamCreateWithFlags(&hp->compute, cudaStreamNonBlocking));
+    EPIC_CUDA_TRY(cudaStreamCreateWithFlags(&hp->copy, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+      EPIC_CUDA_TRY(cudaEventCreateWithFlags(&hp->copied[i], cudaEventDisableTiming));
+      EPIC_CUDA_TRY(cudaEventCreateWithFlags(&hp->consumed[i], cudaEventDisableTiming));
+    }
+  }
+  HostPipe* hp = plan->pipe;
+  if (chunk_bytes > hp->volt_bytes) {
+    EPIC_CUDA_TRY(cudaDeviceSynchronize());
+    for (int i = 0; i < 2; ++i) {
+      if (hp->d_volt[i]) cudaFree(hp->d_volt[i]);
+      hp->d_volt[i] = nullptr;
+    }
+    hp->volt_bytes = 0;
+    for (int i = 0; i < 2; ++i) {
+      const cudaError_t ce = cudaMalloc(&hp->d_volt[i], chunk_bytes);
+      if (ce != cudaSuccess) { set_cuda_error(ce); return ce == cudaErrorMemoryAllocation ? EPIC_ERR_NOMEM : EPIC_ERR_CUDA; }
+    }
+    hp->volt_bytes = chunk_bytes;
+  }
+  if (out_bytes > hp->out_bytes) {
+    EPIC_CUDA_TRY(cudaDeviceSynchronize());
+    if (hp->d_out) cudaFree(hp->d_out);
+    hp->d_out = nullptr;
+    hp->out_bytes = 0;
+    const cudaError_t ce = cudaMalloc(&hp->d_out, out_bytes);
+    if (ce != cudaSuccess) { set_cuda_error(ce); return ce == cudaErrorMemoryAllocation ? EPIC_ERR_NOMEM : EPIC_ERR_CUDA; }
+    hp->out_bytes = out_bytes;
+  }
+  return EPIC_OK;
+}
+
 } // namespace epic
 
 using namespace epic;
@@ -379,6 +434,7 @@ int epic_plan_create_per_channel(epic_plan** out, int grid_n, int pad, int n_ant
   p->d_wide = nullptr;
   p->wide_ok = 0;
   p->stream_k = 0;
+  p->pipe = nullptr;
   p->d_auto = nullptr;
   p->input_order = EPIC_ORDER_TCPA;
   p->ph_n_chan = p->ph_n_pol = 0;
@@ -434,6 +490,7 @@ int epic_plan_destroy(epic_plan* plan) {
   wide_plan_free(plan);
   tiled_plan_free(plan);
   autocorr_plan_free(plan);
+  host_pipe_free(plan);
   if (plan->d_phasor) cudaFree(plan->d_phasor);
   if (plan->d_phasor_pair) cudaFree(plan->d_phasor_pair);
   if (plan->d_scratch) cudaFree(plan->d_scratch);
@@ -524,6 +581,60 @@ int epic_plan_set_path(epic_plan* plan, int path) {
 int epic_image(epic_plan* plan, const void* voltages, int n_t, int n_chan, int n_pol,
                float* out_accum, epic_stream stream) {
   return image_common(plan, voltages, 0, n_t, n_chan, n_pol, out_accum, stream);
+}
+
+int epic_image_host(epic_plan* plan, const void* voltages_host, int n_t, int n_chan, int n_pol,
+                    float* out_accum_host, int accumulate, int n_chunks) {
+  if (!plan) return EPIC_ERR_ARG;
+  if (n_t < 0 || n_chan < 0) return EPIC_ERR_ARG;
+  if (n_pol != 1 && n_pol != 2) return EPIC_ERR_RANGE;
+  const int n_planes = planes_for(n_pol, resolve_products(plan, n_pol));
+  if (n_planes < 0) return EPIC_ERR_RANGE;
+  plan->last_launches = 0;
+  if (plan->n_layout > 1 && n_chan != plan->n_layout) return EPIC_ERR_ARG;
+  if (n_chan == 0) return EPIC_OK;
+  if (!out_accum_host || (n_t > 0 && !voltages_host)) return EPIC_ERR_ARG;
+  const size_t sample_bytes = (size_t)n_chan * n_pol * plan->n_ant;  // one time sample of all channels
+  const size_t out_bytes = (size_t)n_chan * n_planes * plan->N * plan->N * sizeof(float);
+  if (n_chunks <= 0) n_chunks = 4;
+  n_chunks = std::max(1, std::min(n_chunks, n_t));
+  // chunk edges: a short first chunk (its copy is the one nothing can hide), the rest equal
+  std::vector<int> edge(1, 0);
+  const int first = (n_chunks > 1 && n_t >= 4 * n_chunks) ? n_t / (2 * n_chunks) : 0;
+  if (first) edge.push_back(first);
+  const int rest = n_chunks - (first ? 1 : 0);
+  for (int k = 1; k <= rest; ++k) edge.push_back(first + (int)((long long)(n_t - first) * k / rest));
+  int chunk_max = 0;
+  for (size_t k = 0; k + 1 < edge.size(); ++k) chunk_max = std::max(chunk_max, edge[k + 1] - edge[k]);
+  int st = host_pipe_prepare(plan, std::max<size_t>(16, (size_t)chunk_max * sample_bytes), out_bytes);
+  if (st != EPIC_OK) return st;
+  HostPipe* hp = plan->pipe;
+  if (accumulate) EPIC_CUDA_TRY(cudaMemcpyAsync(hp->d_out, out_accum_host, out_bytes, cudaMemcpyHostToDevice, hp->compute));
+  else EPIC_CUDA_TRY(cudaMemsetAsync(hp->d_out, 0, out_bytes, hp->compute));
+  int launches = 0;
+  const uint8_t* src = static_cast<const uint8_t*>(voltages_host);
+  for (size_t k = 0; k + 1 < edge.size(); ++k) {
+    const int a = edge[k], b = edge[k + 1], buf = (int)(k & 1);
+    if (b == a) continue;
+    if (k >= 2) EPIC_CUDA_TRY(cudaStreamWaitEvent(hp->copy, hp->consumed[buf], 0));  // the kernels that read this buffer are done
+    EPIC_CUDA_TRY(cudaMemcpyAsync(hp->d_volt[buf], src + (size_t)a * sample_bytes, (size_t)(b - a) * sample_bytes,
+                                  cudaMemcpyHostToDevice, hp->copy));
+    EPIC_CUDA_TRY(cudaEventRecord(hp->copied[buf], hp->copy));
+    EPIC_CUDA_TRY(cudaStreamWaitEvent(hp->compute, hp->copied[buf], 0));
+    st = image_common(plan, hp->d_volt[buf], 0, b - a, n_chan, n_pol, hp->d_out, hp->compute);
+    if (st != EPIC_OK) break;
+    launches += plan->last_launches;
+    EPIC_CUDA_TRY(cudaEventRecord(hp->consumed[buf], hp->compute));
+  }
+  if (st == EPIC_OK) EPIC_CUDA_TRY(cudaMemcpyAsync(out_accum_host, hp->d_out, out_bytes, cudaMemcpyDeviceToHost, hp->compute));
+  const cudaError_t c1 = cudaStreamSynchronize(hp->copy), c2 = cudaStreamSynchronize(hp->compute);
+  if (st != EPIC_OK) return st;
+  if (c1 != cudaSuccess || c2 != cudaSuccess) {
+    set_cuda_error(c1 != cudaSuccess ? c1 : c2);
+    return EPIC_ERR_CUDA;
+  }
+  plan->last_launches = launches;
+  return EPIC_OK;
 }
 
 int epic_image_cf32(epic_plan* plan, const void* voltages_cf32, int n_t, int n_chan, int n_pol,

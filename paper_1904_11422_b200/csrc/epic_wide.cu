@@ -30,7 +30,7 @@ namespace {
 
 
 // column fold: z[bitrev(y)] = in[y] + c32 in[y+32] + c16 (in[y+16] + c32 in[y+48]); rows y+32 exist while
-// y < NB2, rows y+48 while y < NB3 (RA = 32: neither, 48: NB2 = 16, 64: both)
+// y < NB2, rows y+48 while y < NB3 (RA = 32: neither, 40: NB2 = 8, 48: NB2 = 16, 64: both)
 __device__ __forceinline__ void cmac(float2& sr, float2& si, float2 br, float2 bi, float cr, float ci) {
   sr = __ffma2_rn(br, f2(cr), sr); sr = __ffma2_rn(neg2(bi), f2(ci), sr);
   si = __ffma2_rn(bi, f2(cr), si); si = __ffma2_rn(br, f2(ci), si);
@@ -148,11 +148,11 @@ __device__ __forceinline__ void gather_wide(const FusedParams& P, const float4* 
   }
 }
 
-// RA: rows allocated per plane (32, 48 or 64 >= R; rows R .. RA-1 stay zero); FW: pairs per batch
+// RA: rows allocated per plane (32, 40, 48 or 64 >= R; rows R .. RA-1 stay zero); FW: pairs per batch
 template <int Q, int NPROD, int RA, int FW>
 __global__ void __launch_bounds__(64 * Q, 2) epic_wide_kernel(FusedParams P) {
   constexpr int NT = 64 * Q, N = 32 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1), PLW = RA * HS;
-  constexpr int NB2 = RA > 32 ? 16 : 0, NB3 = RA > 48 ? 16 : 0;
+  constexpr int NB2 = RA > 32 ? (RA - 32 < 16 ? RA - 32 : 16) : 0, NB3 = RA > 48 ? 16 : 0;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* gh = reinterpret_cast<float4*>(smem_raw);  // [FW][RA][HS]
   float4* tws = gh + FW * PLW;                       // [2Q][TWV]
@@ -300,7 +300,7 @@ struct WideTables {
   float4* tw;           // [2Q][TWV] TwSets with the second fold constant r^32 in word 4
   uint16_t* ent_ant;    // gather entries re-ordered by folded cell: (y, x) entries, then (y, x + 32) entries
   float2* ent_tap;
-  int ra;               // rows allocated per plane: 32, 48 or 64
+  int ra;               // rows allocated per plane: 32, 40, 48 or 64
 };
 
 template <int Q>
@@ -332,6 +332,7 @@ int launch_wide(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
 template <int Q, int NPROD>
 int launch_wide_ra(const epic_plan* p, const FusedParams& P, int ra, int fw, cudaStream_t s) {
   if (ra == 32) return launch_wide<Q, NPROD, 32, 4>(p, P, s);
+  if (ra == 40) return fw == 3 ? launch_wide<Q, NPROD, 40, 3>(p, P, s) : launch_wide<Q, NPROD, 40, 2>(p, P, s);
   if (ra == 48) return fw == 3 ? launch_wide<Q, NPROD, 48, 3>(p, P, s) : launch_wide<Q, NPROD, 48, 2>(p, P, s);
   return launch_wide<Q, NPROD, 64, 2>(p, P, s);
 }
@@ -366,7 +367,7 @@ int wide_plan_init(epic_plan* p) {
   if (p->R > 2 * S || p->Cc > 2 * S) return EPIC_OK;
   if (p->R <= S && p->Cc <= S) return EPIC_OK;  // the 32 x 32 kernel takes it
   if (p->h_ent_ant.size() >= ((size_t)1 << 24)) return EPIC_OK;
-  const int R = p->R, ra = R <= 32 ? 32 : (R <= 48 ? 48 : 64);
+  const int R = p->R, ra = R <= 32 ? 32 : (R <= 40 ? 40 : (R <= 48 ? 48 : 64));
   const size_t n_slots = (size_t)R * S;
   std::vector<uint2> info;
   std::vector<uint16_t> ent_ant;

@@ -720,3 +720,39 @@ def test_tensor_core_path_full_size_c2_sampled_channels():
     assert np.isfinite(gpu).all() and (gpu >= 0).all()
     totals = gpu[:, 0].sum(axis=(1, 2))
     assert totals.min() > 0.5 * totals.max()
+
+
+# ------------------------------------------------------------------ host-buffer entry point
+@pytest.mark.parametrize("wl,chunks", [
+    (make_config(2, n_chan=5, n_t=41), 4),                 # fused, chunks of unequal length
+    (make_config(3, n_chan=3, n_t=16), 0),                 # default chunking, four products
+    (make_lwa55(n_chan=2, n_t=9), 16),                     # wide kernel, more chunks than samples allow
+    (make_config(4, n_chan=2, n_t=6), 2),                  # large grid
+    (make_custom(grid_n=8, pad=2, n_ant=30, n_pol=2, kernel_k=3, n_chan=2, n_t=5, layout="wrap"), 1),  # two-pass, one chunk
+], ids=lambda v: v.name if hasattr(v, "name") else str(v))
+def test_image_host_matches_oracle_and_accumulates(wl, chunks):
+    """epic_image_host: HOST voltages in, HOST images out, the copies pipelined inside the library; pageable numpy
+    memory and pinned torch memory, overwrite and accumulate modes."""
+    import torch
+    epic = _epic()
+    v = wl.voltages()
+    ref = run_oracle(wl, volt=v)
+    with epic.Plan(wl.grid_n, wl.pad, wl.ant_uv, wl.taps, wl.kernel_k) as plan:
+        plan.set_products(wl.n_products)
+        shape = (wl.n_chan, plan.n_planes(wl.n_pol), wl.N, wl.N)
+        out = np.full(shape, 7.0, dtype=np.float32)                      # pageable; overwritten
+        plan.image_host(v, wl.n_t, wl.n_chan, wl.n_pol, out, accumulate=False, n_chunks=chunks)
+        assert plan.last_launches() > 0
+        assert_parity(out, ref, what=f"{wl.name} host, overwrite")
+        hv = torch.from_numpy(v).pin_memory()
+        hout = torch.from_numpy(out.copy()).pin_memory()
+        half = wl.n_t // 2
+        plan.image_host(hv[half:].contiguous().pin_memory(), wl.n_t - half, wl.n_chan, wl.n_pol, hout, accumulate=True, n_chunks=chunks)
+        second = run_oracle(wl, volt=v[half:])
+        assert_parity(hout.numpy(), ref + second, what=f"{wl.name} host, accumulate")
+        plan.image_host(v, 0, wl.n_chan, wl.n_pol, out, accumulate=True)  # empty gulp: unchanged
+        assert_parity(out, ref, what="empty gulp")
+        with pytest.raises(ValueError):
+            plan.image_host(v[:, :, :, ::2], wl.n_t, wl.n_chan, wl.n_pol, out)      # non-contiguous
+        with pytest.raises(ValueError):
+            plan.image_host(v, wl.n_t + 1, wl.n_chan, wl.n_pol, out)                # too short
