@@ -199,6 +199,22 @@ def test_wide_support_plans_both_paths(wl, path):
                 plan.set_path(epic.EPIC_PATH_TENSOR)   # the tensor-core variant is the 32 x 32 kernel's
 
 
+@pytest.mark.parametrize("kernel,n_products,channels", [("tophat", 4, [3, 90]), ("delta", 2, [0, 64, 127])], ids=["tophat", "delta"])
+def test_wide_full_size_sampled_channels(kernel, n_products, channels):
+    """The paper's operating point at C2's extent (128 channels x 1000 samples), in the launch configuration
+    `bench.py --workload lwa55-*` and the default run's other_configs time (one call, AUTO = the wide fused kernel);
+    whole channels against the oracle, properties for the rest."""
+    wl = make_lwa55(n_chan=128, n_t=1000, kernel=kernel, n_products=n_products)
+    v = wl.voltages()
+    gpu, info = run_gpu(wl, volt=v, return_plan_info=True)
+    assert info["path"] == 2 and info["launches"] == 2 and max(info["support"][2:]) > 32
+    ref = run_oracle(wl, volt=v, channels=channels)
+    assert_parity(gpu[channels], ref, what=f"{wl.name} channels {channels}")
+    assert np.isfinite(gpu).all() and (gpu[:, :2] >= 0).all()
+    totals = gpu[:, 0].sum(axis=(1, 2))
+    assert totals.min() > 0.5 * totals.max()
+
+
 @pytest.mark.parametrize("mode", ["native", "phasors", "both"])
 def test_wide_input_order_and_delay_phasors(mode):
     wl = make_lwa55(n_chan=2, n_t=7)
