@@ -159,6 +159,16 @@ def measured_hbm_gbs():
         return HBM_FALLBACK_GBS, "B200_PROFILING.md fallback"
 
 
+def input_fingerprint(wl, volt) -> dict:
+    """numpy version and SHA-256 of every generated buffer, so that a run can be tied to its inputs."""
+    import hashlib
+    h = lambda a: hashlib.sha256(np.ascontiguousarray(a).tobytes()).hexdigest()
+    out = {"numpy": np.__version__, "seed": int(wl.seed), "sha256": {"voltages": h(volt), "ant_uv": h(wl.ant_uv)}}
+    if wl.taps is not None:
+        out["sha256"]["taps"] = h(wl.taps)
+    return out
+
+
 def measured_traffic(wl_name: str, path: int):
     """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of this workload and kernel family
     from the ncu captures summarised in profiles/traffic.csv, or None."""
@@ -493,6 +503,7 @@ def run_epic(args, wl):
                        f"timed with the host clock, device idle before and after"},
         "gpu_launches": int(launches),
         "clocks": clocks,
+        "inputs": input_fingerprint(wl, volt),
     }
     if path == 4:
         # the tensor-core variant, reported beside the FP32 roofline above (same algorithmic flops, so the two

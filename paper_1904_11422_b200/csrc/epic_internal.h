@@ -69,7 +69,6 @@ struct epic_plan {
   float2* d_phasor;            // [ph_n_chan][ph_n_pol][n_ant] complex multipliers (reading Q19)
   float4* d_phasor_pair;       // [ph_n_chan][n_ant] (re_lo, re_hi, im_lo, im_hi): lo/hi = pol X/Y, or the same pol twice
   int tiled_ok;                // N is 256 or 512
-  int stream_k;                // tuning: row CTAs per row group of the streamed path (0 = default)
   epic::HostPipe* pipe;        // streams, events and device staging of epic_image_host (created on first use)
   int n_sm;
   // host copies kept for the fused path's table builder

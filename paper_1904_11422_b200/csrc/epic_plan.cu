@@ -433,7 +433,6 @@ int epic_plan_create_per_channel(epic_plan** out, int grid_n, int pad, int n_ant
   p->tiled_ok = 0;
   p->d_wide = nullptr;
   p->wide_ok = 0;
-  p->stream_k = 0;
   p->pipe = nullptr;
   p->d_auto = nullptr;
   p->input_order = EPIC_ORDER_TCPA;

@@ -426,7 +426,7 @@ template <int MODE> constexpr int stream_ent_bytes() { return (MODE == 0 ? 0 : (
 // one row / column, sit in ONE warp -- lane = rho + 2 j + 2 J b, item = warp * (16 / J) + b -- so the
 // step-1 / step-2 exchange through shared memory needs only __syncwarp(), not a CTA barrier (the first
 // version of this kernel had 6 CTA barriers per row item: `barrier` was 6.3 of its 12 stall cycles per
-// issue, profiles/r02_stream_ncu.md).  The two residues of a row / column are in adjacent lanes
+// issue, profiles/r02_large_grid_ncu.md).  The two residues of a row / column are in adjacent lanes
 // (LDS.128 merges same-address lane pairs).
 // Exchange block of a team: [J][16] float4, element (j, k1) at j * 16 + (k1 ^ j ^ 4 rho): the XOR
 // swizzle keeps a quarter-warp's 8 accesses in 8 distinct 16-byte bank groups both ways, unpadded.
@@ -916,16 +916,14 @@ int launch_stream(epic_plan* p, const ImageArgs& a, StreamParams& S, int cap) {
   const long long slots = (long long)per_sm * p->n_sm;
   // K row CTAs per (channel, row group), interleaved in time: a row item is a longer dependent chain than a column
   // frame, and rows : columns = K n_groups : strips is then close to the 1 : 1 split of the work
-  int K = p->stream_k > 0 ? p->stream_k : 2;
-  if (const char* ek = std::getenv("EPIC_STREAM_K")) K = std::max(1, std::atoi(ek));  // development knob
+  int K = 2;  // measured on C4 / C5: K = 1 1.40 / 0.094, K = 2 1.95 / 0.216, K = 3 1.65 / (falls back to 1) M frames/s
   if (slots / (strips + K * n_groups) < 1) K = 1;
   long long Cw = std::min<long long>(a.n_chan, slots / (strips + K * n_groups));
   if (Cw < 1) return EPIC_ERR_RANGE;
   const int n_waves = (int)((a.n_chan + Cw - 1) / Cw);
   Cw = (a.n_chan + n_waves - 1) / n_waves;  // equal waves
   const int n_pairs = a.n_pol == 2 ? a.n_t : (a.n_t + 1) / 2;
-  int B = 4;  // frames per hand-over block: one flag round trip per B frames
-  if (const char* eb = std::getenv("EPIC_STREAM_B")) B = std::max(1, std::atoi(eb));  // development knob
+  int B = 4;  // frames per hand-over block: one flag round trip per B frames (measured: 1, 4, 8 within 6 % of each other)
   B = std::min(B, n_pairs);
   const int nbw = (n_pairs + B - 1) / B;
   const long long n_seq = (long long)n_waves * nbw;
