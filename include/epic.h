@@ -115,7 +115,7 @@ EPIC_API int epic_plan_set_products(epic_plan* plan, int n_products);
 EPIC_API int epic_plan_set_path(epic_plan* plan, int path);
 
 /* Tuning: bytes of the plan's scratch (the intermediate H of the tiled / two-pass paths) one batch may
- * use; 0 = all of it (1 GiB for N >= 256, else 64 MiB).  A small limit (e.g. 64 MiB) keeps H resident in
+ * use; 0 = all of it (1 GiB for N >= 256, else 128 MiB).  A small limit (e.g. 64 MiB) keeps H resident in
  * the 126 MB L2 at the price of more, shorter batches, each ending in one read-modify-write of its
  * channels' out_accum.  A batch always holds at least one frame. */
 EPIC_API int epic_plan_set_scratch_limit(epic_plan* plan, long long bytes);

@@ -222,6 +222,187 @@ epic_fused_kernel(FusedParams P) {
 }
 
 
+// ================================================================ dual-residue variant (four products, tap kernels)
+// The Q residue CTAs of a channel each repeat the whole gather (C3: 28 % of warp time, DRAM 2.2x algorithmic).
+// Here one CTA runs TWO column residues l2 = 2u, 2u + 1 from ONE gather: per batch of F2 = 2 pairs it grids once,
+// row-transforms every row twice (the four tasks (h, residue) of a row sit in adjacent lanes: both residues load
+// the gathered row, __syncwarp, residue 0 stores in place and residue 1 into a second plane set), and runs the
+// column pass + products for residue 0 and then residue 1, each with its own accumulators in tensor memory
+// (2 x 64 columns per thread).  Per frame and residue the gather work halves; everything else is unchanged:
+// 4 column tasks per thread and batch, the same table-read amortisation (2 frames x 2 residues), two CTAs per SM.
+constexpr int F2 = 2;  // pairs per batch
+
+template <int NB>
+__device__ __forceinline__ void row_task_dual(const float4* __restrict__ src, float4* __restrict__ dst,
+                                              const float4* __restrict__ tw, int h, bool valid) {
+  C2 z[16];
+  transform32<NB>(z, src, 1, tw);
+  __syncwarp();  // both residues (and both h) of the row have loaded it: residue 0 may overwrite it
+  if (valid) {
+#pragma unroll
+    for (int k = 0; k < 16; ++k) dst[2 * k + h] = make_float4(z[k].re.x, z[k].re.y, z[k].im.x, z[k].im.y);
+  }
+}
+
+// partial sums of split units, as epic_fused_fixup, for units of two residues: [cta][slot][residue][4][16][NT]
+template <int Q>
+__global__ void __launch_bounds__(64 * Q) epic_fused_dual_fixup(FusedParams P, int main_grid) {
+  constexpr int NT = 64 * Q, KPT = 16, N = 32 * Q, NACC = 4;
+  const int unit = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const long long G = main_grid, first = (long long)unit * P.nb, last = first + P.nb - 1;
+  const int b_lo = (int)(((first + 1) * G - 1) / P.total), b_hi = (int)(((last + 1) * G - 1) / P.total);
+  if (b_lo == b_hi) return;  // the unit ran in one CTA and was added directly
+  const int l1 = (warp & 1) * 16 + (lane >> 1);
+  const int rho = (warp >> 1) * 2 + (lane & 1);
+  const int c = unit / (Q / 2), u2 = unit - c * (Q / 2);
+  const size_t plane = (size_t)N * N;
+  for (int res = 0; res < 2; ++res) {
+    float* o = P.out + (size_t)c * P.n_planes * plane + (Q * l1 + 2 * u2 + res) + (size_t)rho * N;
+    for (int k = 0; k < KPT; ++k) {
+      float v[NACC] = {0.0f, 0.0f, 0.0f, 0.0f};
+      for (int b = b_lo; b <= b_hi; ++b) {
+        const int slot = (first <= P.total * b / G) ? 0 : 1;
+        const float* part = P.partial + ((size_t)((b * 2 + slot) * 2 + res) * NACC * KPT) * NT + tid;
+#pragma unroll
+        for (int q = 0; q < NACC; ++q) v[q] += part[(size_t)(q * KPT + k) * NT];
+      }
+      add_pixel<4>(o + (size_t)k * 2 * Q * N, plane, v);
+    }
+  }
+}
+
+template <int Q, int NB, bool STG>
+__global__ void __launch_bounds__(64 * Q, 2) epic_fused_dual_kernel(FusedParams P) {
+  constexpr int NT = 64 * Q, N = 32 * Q, HQ = Q / 2;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float4* gA = reinterpret_cast<float4*>(smem_raw);  // [F2][32][HS] gridded planes, then residue 0's rows (in place)
+  float4* gB = gA + F2 * PLANE;                      // [F2][32][HS] residue 1's rows
+  float4* tws = gB + F2 * PLANE;                     // [2Q][TWV]
+  float4* E = tws + 2 * Q * TWV;                     // [F2][A]
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+  const long long g0 = P.total * (long long)blockIdx.x / gridDim.x;
+  const long long g1 = P.total * (long long)(blockIdx.x + 1) / gridDim.x;
+  if (g0 >= g1) return;
+  constexpr int TCOLS1 = Q == 4 ? 128 : 64, TCOLS = 2 * TCOLS1;  // one block of accumulator columns per residue
+
+  int unit = (int)(g0 / P.nb);  // unit = (channel, residue pair)
+  uint2 info[S * S / NT];
+#pragma unroll
+  for (int j = 0; j < S * S / NT; ++j) info[j] = __ldg(P.cell_info + tid + j * NT);
+  for (int i = tid; i < 2 * F2 * PLANE; i += NT) gA[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);  // rows >= R stay zero
+  for (int i = tid; i < 2 * Q * TWV; i += NT) tws[i] = __ldg(P.tw + i);
+  float2* tap_s = reinterpret_cast<float2*>(E + F2 * P.n_ant);
+  uint16_t* ant_s = reinterpret_cast<uint16_t*>(tap_s + P.n_ent);
+  if constexpr (STG) {
+    for (int i = tid; i < P.n_ent; i += NT) { tap_s[i] = __ldg(P.ent_tap + i); ant_s[i] = __ldg(P.ent_ant + i); }
+  }
+  __syncthreads();
+
+  const int l1 = (warp & 1) * 16 + (lane >> 1);
+  const int rho = (warp >> 1) * 2 + (lane & 1);
+  __shared__ uint32_t tmem_slot;
+  const uint32_t tbase = tmem_alloc_cta<TCOLS>(&tmem_slot, warp);
+  const uint32_t taddr = tbase + (((uint32_t)(warp & 3) * 32u) << 16) + (uint32_t)(warp >> 2) * 64u;
+  {
+    float zero[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) zero[i] = 0.0f;
+#pragma unroll
+    for (int res = 0; res < 2; ++res)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) tmem_st16(taddr + res * TCOLS1 + 16 * c, zero);
+    tmem_wait_st();
+  }
+
+  // S6, as in epic_fused_kernel, for both residues of the unit
+  auto flush = [&](int unit, bool complete, int slot) {
+    const int c = unit / HQ, u2 = unit - c * HQ;
+    const size_t plane = (size_t)N * N;
+#pragma unroll 1
+    for (int res = 0; res < 2; ++res) {
+      float* o = P.out + (size_t)c * P.n_planes * plane + (Q * l1 + 2 * u2 + res);
+      float* part = P.partial + ((size_t)((blockIdx.x * 2 + slot) * 2 + res) * 4 * 16) * NT + tid;
+      const uint32_t ta = taddr + res * TCOLS1;
+#pragma unroll
+      for (int c4 = 0; c4 < 4; ++c4) {
+        float a[16], zero[16];
+        tmem_ld16(ta + 16 * c4, a);
+#pragma unroll
+        for (int i = 0; i < 16; ++i) zero[i] = 0.0f;
+        tmem_st16(ta + 16 * c4, zero);
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk) {
+          const int k = 4 * c4 + kk;
+          const float v[4] = {a[4 * kk], a[4 * kk + 1], a[4 * kk + 2], a[4 * kk + 3]};
+          if (complete) {
+            add_pixel<4>(o + (size_t)(2 * Q * k + rho) * N, plane, v);
+          } else {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) part[(size_t)(q * 16 + k) * NT] = v[q];
+          }
+        }
+      }
+      tmem_wait_st();
+    }
+  };
+
+  int b = (int)(g0 - (long long)unit * P.nb);
+  const int first_unit = unit;
+  int seg_begin = b;
+  PrefetchSlots ps;
+  prefetch_init<NT, F2>(P, tid, ps);
+  uint32_t wlo[MAXW], whi[MAXW];
+  prefetch_batch<NT, F2>(P, ps, unit / HQ, b, wlo, whi);
+  unpack_batch<false>(P, ps, E, wlo, whi, unit / HQ);
+  __syncthreads();
+
+  const int ntask = F2 * P.R * 4;  // (pair, row, h, residue), residue fastest: a row's four tasks are adjacent lanes
+  for (long long g = g0; g < g1; ++g) {
+    int unit_n = unit, b_n = b + 1;
+    if (b_n == P.nb) { b_n = 0; ++unit_n; }
+    const bool more = g + 1 < g1;
+    if (more) prefetch_batch<NT, F2>(P, ps, unit_n / HQ, b_n, wlo, whi);
+
+    gather_batch<NT, false, STG, false, F2>(P, E, gA, info, ant_s, tap_s);
+    __syncthreads();
+
+    const int l2a = 2 * (unit % HQ);
+    for (int base = warp * 32; base < ntask; base += NT) {
+      const int task = base + lane;
+      const bool valid = task < ntask;
+      // idle lanes transform the all-zero row 31 of plane 0 (they exist only when R < 32)
+      int f = 0, y = S - 1, h = 0, res = 0;
+      if (valid) { res = task & 1; h = (task >> 1) & 1; const int p = task >> 2; f = p / P.R; y = p - f * P.R; }
+      const float4* src = gA + f * PLANE + y * HS;
+      row_task_dual<NB>(src, (res ? gB : gA) + f * PLANE + y * HS, tws + (l2a + res + Q * h) * TWV, h, valid);
+    }
+    __syncthreads();
+
+    if (more) unpack_batch<false>(P, ps, E, wlo, whi, unit_n / HQ);  // E was last read by this batch's gather
+#pragma unroll 1
+    for (int rf = 0; rf < 2 * F2; ++rf) {
+      const int res = rf / F2, f = rf - res * F2;
+      int tw_off = rho * TWV;
+      asm volatile("" : "+r"(tw_off));
+      col_task_tmem<NB>((res ? gB : gA) + f * PLANE + l1, tws + tw_off, taddr + res * TCOLS1);
+    }
+
+    if (unit_n != unit || !more) {
+      flush(unit, seg_begin == 0 && b == P.nb - 1, unit == first_unit ? 0 : 1);
+      seg_begin = 0;
+    }
+    unit = unit_n; b = b_n;
+    __syncthreads();  // next batch's E is complete; the planes are free
+  }
+  tmem_free_cta<TCOLS>(tbase, warp);
+}
+
+template <int Q>
+size_t fused_dual_smem_bytes(int n_ant) {
+  return ((size_t)2 * F2 * PLANE + (size_t)2 * Q * TWV + (size_t)F2 * n_ant) * sizeof(float4);
+}
+
 // ================================================================ tensor-core column pass
 // The column transform of a unit is a dense contraction: A[m][(f, pol, l1)] = sum_y F[m][y] H[y][(f, pol, l1)],
 // F[m][y] = exp(+2 pi i m y / N) (128 x 32), H = the row-pass output of the batch (32 x 256).  Here it
@@ -518,10 +699,39 @@ int launch_fused(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
   return EPIC_OK;
 }
 
+// dual-residue kernel (four products, tap gather, one layout): sized for two CTAs per SM
+template <int Q, int NB, bool STG>
+int launch_fused_dual(const epic_plan* p, FusedParams P, cudaStream_t s) {
+  constexpr int NT = 64 * Q;
+  P.pairs_per_batch = F2;
+  P.nb = (P.n_t + F2 - 1) / F2;
+  P.total = (long long)P.n_chan * (Q / 2) * P.nb;
+  const size_t smem = fused_dual_smem_bytes<Q>(P.n_ant) + (STG ? fused_stage_bytes(P.n_ent) : 0);
+  auto kern = epic_fused_dual_kernel<Q, NB, STG>;
+  if (smem > 48 * 1024)
+    EPIC_CUDA_TRY(cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  // tensor-memory kernels: the occupancy query answers 1; two CTAs (2 x 256 of the 512 columns for Q = 4) share an SM
+  const int per_sm = 2 * (smem + 1024) <= (size_t)227 * 1024 ? 2 : 1;
+  const int grid = (int)std::min<long long>(P.total, (long long)per_sm * p->n_sm);
+  if ((size_t)grid * 2 * 2 * 4 * 16 * NT * sizeof(float) > p->scratch_bytes) return EPIC_ERR_RANGE;
+  kern<<<grid, NT, smem, s>>>(P);
+  epic_fused_dual_fixup<Q><<<(unsigned)(P.total / P.nb), NT, 0, s>>>(P, grid);
+  EPIC_CUDA_TRY(cudaGetLastError());
+  return EPIC_OK;
+}
+
 template <int Q, int NPROD, bool DELTA>
 int launch_fused_nb(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
   // elements y + 16 of a row/column are read only while y < NB (the rest of the block is empty)
   const bool pc = P.cell_stride != 0, nb12 = std::max(p->R, p->Cc) <= 16 + 12;
+  if constexpr (!DELTA && NPROD == 4) {  // two residues per CTA from one gather (needs the scratch for its partial sums)
+    if (!pc && (size_t)2 * p->n_sm * 2 * 2 * 4 * 16 * 64 * Q * sizeof(float) <= p->scratch_bytes) {
+      const bool stg = 2 * (fused_dual_smem_bytes<Q>(P.n_ant) + fused_stage_bytes(P.n_ent) + 1024 + 128) <= (size_t)227 * 1024;
+      if (stg) return nb12 ? launch_fused_dual<Q, 12, true>(p, P, s) : launch_fused_dual<Q, 16, true>(p, P, s);
+      if (2 * (fused_dual_smem_bytes<Q>(P.n_ant) + 1024 + 128) <= (size_t)227 * 1024)
+        return nb12 ? launch_fused_dual<Q, 12, false>(p, P, s) : launch_fused_dual<Q, 16, false>(p, P, s);
+    }
+  }
   if constexpr (!DELTA) {  // staged gather tables, if two CTAs still fit an SM with them
     if (!pc && 2 * (fused_smem_bytes<Q>(P.n_ant) + fused_stage_bytes(P.n_ent) + 1024 + 128) <= (size_t)227 * 1024)
       return nb12 ? launch_fused<Q, NPROD, DELTA, 12, false, true>(p, P, s)

@@ -462,7 +462,7 @@ int epic_plan_create_per_channel(epic_plan** out, int grid_n, int pad, int n_ant
     // path's partial sums.  Large planes get 1 GiB: a batch then spans ~150 time samples per channel,
     // which amortises the per-batch read-modify-write of out_accum (measured: C4 +30 % over 96 MiB).
     const size_t frame = (size_t)2 * p->R * p->N * sizeof(float2);
-    const size_t want = p->N >= 256 ? ((size_t)1 << 30) : ((size_t)64 << 20);
+    const size_t want = p->N >= 256 ? ((size_t)1 << 30) : ((size_t)128 << 20);
     p->scratch_bytes = std::max(want, frame);
     ce = cudaMalloc(&p->d_scratch, p->scratch_bytes);
     if (ce != cudaSuccess) {
