@@ -39,6 +39,7 @@
 //   the partial-sum fix-up kernel when the unit's time range was split between two CTAs).
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <type_traits>
 #include <vector>
@@ -244,10 +245,35 @@ __device__ __forceinline__ void row_task_dual(const float4* __restrict__ src, fl
   }
 }
 
+// one or two products: accumulators (|A_lo|^2, |A_hi|^2) of a thread's 16 pixels in 32 columns of tensor memory
+template <int NB>
+__device__ __forceinline__ void col_task_tmem2(const float4* __restrict__ col, const float4* __restrict__ tw, uint32_t taddr) {
+  C2 z[16];
+  uint32_t r[2][16];
+  tmem_ld16_issue(taddr, r[0]);  // the first 8 pixels' accumulators travel during the transform
+  transform32<NB>(z, col, HS, tw);
+#pragma unroll
+  for (int c = 0; c < 2; ++c) {
+    tmem_wait_ld();
+    if (c == 0) tmem_ld16_issue(taddr + 16, r[1]);  // the other 8, during this update
+    float a[16];
+#pragma unroll
+    for (int kk = 0; kk < 8; ++kk) {
+      const C2& v = z[8 * c + kk];
+      float2 p = make_float2(__uint_as_float(r[c][2 * kk]), __uint_as_float(r[c][2 * kk + 1]));
+      p = __ffma2_rn(v.re, v.re, p);
+      p = __ffma2_rn(v.im, v.im, p);
+      a[2 * kk] = p.x; a[2 * kk + 1] = p.y;
+    }
+    tmem_st16(taddr + 16 * c, a);
+  }
+  tmem_wait_st();
+}
+
 // partial sums of split units, as epic_fused_fixup, for units of two residues: [cta][slot][residue][4][16][NT]
-template <int Q>
+template <int Q, int NPROD>
 __global__ void __launch_bounds__(64 * Q) epic_fused_dual_fixup(FusedParams P, int main_grid) {
-  constexpr int NT = 64 * Q, KPT = 16, N = 32 * Q, NACC = 4;
+  constexpr int NT = 64 * Q, KPT = 16, N = 32 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
   const int unit = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const long long G = main_grid, first = (long long)unit * P.nb, last = first + P.nb - 1;
   const int b_lo = (int)(((first + 1) * G - 1) / P.total), b_hi = (int)(((last + 1) * G - 1) / P.total);
@@ -259,38 +285,45 @@ __global__ void __launch_bounds__(64 * Q) epic_fused_dual_fixup(FusedParams P, i
   for (int res = 0; res < 2; ++res) {
     float* o = P.out + (size_t)c * P.n_planes * plane + (Q * l1 + 2 * u2 + res) + (size_t)rho * N;
     for (int k = 0; k < KPT; ++k) {
-      float v[NACC] = {0.0f, 0.0f, 0.0f, 0.0f};
+      float v[NACC];
+#pragma unroll
+      for (int q = 0; q < NACC; ++q) v[q] = 0.0f;
       for (int b = b_lo; b <= b_hi; ++b) {
         const int slot = (first <= P.total * b / G) ? 0 : 1;
         const float* part = P.partial + ((size_t)((b * 2 + slot) * 2 + res) * NACC * KPT) * NT + tid;
 #pragma unroll
         for (int q = 0; q < NACC; ++q) v[q] += part[(size_t)(q * KPT + k) * NT];
       }
-      add_pixel<4>(o + (size_t)k * 2 * Q * N, plane, v);
+      add_pixel<NPROD>(o + (size_t)k * 2 * Q * N, plane, v);
     }
   }
 }
 
-template <int Q, int NB, bool STG>
+template <int Q, int NPROD, bool DELTA, int NB, bool STG>
 __global__ void __launch_bounds__(64 * Q, 2) epic_fused_dual_kernel(FusedParams P) {
-  constexpr int NT = 64 * Q, N = 32 * Q, HQ = Q / 2;
+  static_assert(!(STG && DELTA), "staged tables: tap kernels only");
+  constexpr int NT = 64 * Q, N = 32 * Q, HQ = Q / 2, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
+  constexpr int CPT = NPROD == 4 ? 64 : 32;  // accumulator columns per thread and residue
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* gA = reinterpret_cast<float4*>(smem_raw);  // [F2][32][HS] gridded planes, then residue 0's rows (in place)
-  float4* gB = gA + F2 * PLANE;                      // [F2][32][HS] residue 1's rows
-  float4* tws = gB + F2 * PLANE;                     // [2Q][TWV]
+  // residue 1's planes are skewed by 4 cells (64 bytes): in the row pass the (h, residue) tasks of two rows make a
+  // quarter-warp, and without the skew the two residues' stores of one row fall in the same 16-byte bank groups
+  // (216 M of 445 M store wavefronts were conflicts before)
+  float4* gB = gA + F2 * PLANE + 4;                  // [F2][32][HS] residue 1's rows
+  float4* tws = gA + 2 * F2 * PLANE + 8;             // [2Q][TWV]
   float4* E = tws + 2 * Q * TWV;                     // [F2][A]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
   const long long g0 = P.total * (long long)blockIdx.x / gridDim.x;
   const long long g1 = P.total * (long long)(blockIdx.x + 1) / gridDim.x;
   if (g0 >= g1) return;
-  constexpr int TCOLS1 = Q == 4 ? 128 : 64, TCOLS = 2 * TCOLS1;  // one block of accumulator columns per residue
+  constexpr int TCOLS1 = (Q == 4 ? 2 : 1) * CPT, TCOLS = 2 * TCOLS1;  // one block of accumulator columns per residue
 
   int unit = (int)(g0 / P.nb);  // unit = (channel, residue pair)
   uint2 info[S * S / NT];
 #pragma unroll
   for (int j = 0; j < S * S / NT; ++j) info[j] = __ldg(P.cell_info + tid + j * NT);
-  for (int i = tid; i < 2 * F2 * PLANE; i += NT) gA[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);  // rows >= R stay zero
+  for (int i = tid; i < 2 * F2 * PLANE + 8; i += NT) gA[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);  // rows >= R stay zero
   for (int i = tid; i < 2 * Q * TWV; i += NT) tws[i] = __ldg(P.tw + i);
   float2* tap_s = reinterpret_cast<float2*>(E + F2 * P.n_ant);
   uint16_t* ant_s = reinterpret_cast<uint16_t*>(tap_s + P.n_ent);
@@ -303,7 +336,7 @@ __global__ void __launch_bounds__(64 * Q, 2) epic_fused_dual_kernel(FusedParams 
   const int rho = (warp >> 1) * 2 + (lane & 1);
   __shared__ uint32_t tmem_slot;
   const uint32_t tbase = tmem_alloc_cta<TCOLS>(&tmem_slot, warp);
-  const uint32_t taddr = tbase + (((uint32_t)(warp & 3) * 32u) << 16) + (uint32_t)(warp >> 2) * 64u;
+  const uint32_t taddr = tbase + (((uint32_t)(warp & 3) * 32u) << 16) + (uint32_t)(warp >> 2) * CPT;
   {
     float zero[16];
 #pragma unroll
@@ -311,35 +344,44 @@ __global__ void __launch_bounds__(64 * Q, 2) epic_fused_dual_kernel(FusedParams 
 #pragma unroll
     for (int res = 0; res < 2; ++res)
 #pragma unroll
-      for (int c = 0; c < 4; ++c) tmem_st16(taddr + res * TCOLS1 + 16 * c, zero);
+      for (int c = 0; c < CPT / 16; ++c) tmem_st16(taddr + res * TCOLS1 + 16 * c, zero);
     tmem_wait_st();
   }
 
-  // S6, as in epic_fused_kernel, for both residues of the unit
+  // S6, as in epic_fused_kernel, for both residues of the unit.  Column layout per thread and residue:
+  // four products 4 k + {XX, YY, Re XY, Im XY}; one or two products 2 k + {lo, hi}
   auto flush = [&](int unit, bool complete, int slot) {
     const int c = unit / HQ, u2 = unit - c * HQ;
     const size_t plane = (size_t)N * N;
 #pragma unroll 1
     for (int res = 0; res < 2; ++res) {
       float* o = P.out + (size_t)c * P.n_planes * plane + (Q * l1 + 2 * u2 + res);
-      float* part = P.partial + ((size_t)((blockIdx.x * 2 + slot) * 2 + res) * 4 * 16) * NT + tid;
+      float* part = P.partial + ((size_t)((blockIdx.x * 2 + slot) * 2 + res) * NACC * 16) * NT + tid;
       const uint32_t ta = taddr + res * TCOLS1;
+      constexpr int PPC = NPROD == 4 ? 4 : 8;  // pixels per 16-column chunk
 #pragma unroll
-      for (int c4 = 0; c4 < 4; ++c4) {
+      for (int c4 = 0; c4 < CPT / 16; ++c4) {
         float a[16], zero[16];
         tmem_ld16(ta + 16 * c4, a);
 #pragma unroll
         for (int i = 0; i < 16; ++i) zero[i] = 0.0f;
         tmem_st16(ta + 16 * c4, zero);
 #pragma unroll
-        for (int kk = 0; kk < 4; ++kk) {
-          const int k = 4 * c4 + kk;
-          const float v[4] = {a[4 * kk], a[4 * kk + 1], a[4 * kk + 2], a[4 * kk + 3]};
+        for (int kk = 0; kk < PPC; ++kk) {
+          const int k = PPC * c4 + kk;
+          float v[NACC];
+          if constexpr (NPROD == 4) {
+            v[0] = a[4 * kk]; v[1] = a[4 * kk + 1]; v[2] = a[4 * kk + 2]; v[3] = a[4 * kk + 3];
+          } else if constexpr (NPROD == 2) {
+            v[0] = a[2 * kk]; v[1] = a[2 * kk + 1];
+          } else {
+            v[0] = a[2 * kk] + a[2 * kk + 1];
+          }
           if (complete) {
-            add_pixel<4>(o + (size_t)(2 * Q * k + rho) * N, plane, v);
+            add_pixel<NPROD>(o + (size_t)(2 * Q * k + rho) * N, plane, v);
           } else {
 #pragma unroll
-            for (int q = 0; q < 4; ++q) part[(size_t)(q * 16 + k) * NT] = v[q];
+            for (int q = 0; q < NACC; ++q) part[(size_t)(q * 16 + k) * NT] = v[q];
           }
         }
       }
@@ -354,7 +396,7 @@ __global__ void __launch_bounds__(64 * Q, 2) epic_fused_dual_kernel(FusedParams 
   prefetch_init<NT, F2>(P, tid, ps);
   uint32_t wlo[MAXW], whi[MAXW];
   prefetch_batch<NT, F2>(P, ps, unit / HQ, b, wlo, whi);
-  unpack_batch<false>(P, ps, E, wlo, whi, unit / HQ);
+  unpack_batch<DELTA>(P, ps, E, wlo, whi, unit / HQ);
   __syncthreads();
 
   const int ntask = F2 * P.R * 4;  // (pair, row, h, residue), residue fastest: a row's four tasks are adjacent lanes
@@ -364,7 +406,7 @@ __global__ void __launch_bounds__(64 * Q, 2) epic_fused_dual_kernel(FusedParams 
     const bool more = g + 1 < g1;
     if (more) prefetch_batch<NT, F2>(P, ps, unit_n / HQ, b_n, wlo, whi);
 
-    gather_batch<NT, false, STG, false, F2>(P, E, gA, info, ant_s, tap_s);
+    gather_batch<NT, DELTA, STG, DELTA, F2>(P, E, gA, info, ant_s, tap_s);
     __syncthreads();
 
     const int l2a = 2 * (unit % HQ);
@@ -379,13 +421,14 @@ __global__ void __launch_bounds__(64 * Q, 2) epic_fused_dual_kernel(FusedParams 
     }
     __syncthreads();
 
-    if (more) unpack_batch<false>(P, ps, E, wlo, whi, unit_n / HQ);  // E was last read by this batch's gather
+    if (more) unpack_batch<DELTA>(P, ps, E, wlo, whi, unit_n / HQ);  // E was last read by this batch's gather
 #pragma unroll 1
     for (int rf = 0; rf < 2 * F2; ++rf) {
       const int res = rf / F2, f = rf - res * F2;
       int tw_off = rho * TWV;
       asm volatile("" : "+r"(tw_off));
-      col_task_tmem<NB>((res ? gB : gA) + f * PLANE + l1, tws + tw_off, taddr + res * TCOLS1);
+      if constexpr (NPROD == 4) col_task_tmem<NB>((res ? gB : gA) + f * PLANE + l1, tws + tw_off, taddr + res * TCOLS1);
+      else col_task_tmem2<NB>((res ? gB : gA) + f * PLANE + l1, tws + tw_off, taddr + res * TCOLS1);
     }
 
     if (unit_n != unit || !more) {
@@ -400,7 +443,7 @@ __global__ void __launch_bounds__(64 * Q, 2) epic_fused_dual_kernel(FusedParams 
 
 template <int Q>
 size_t fused_dual_smem_bytes(int n_ant) {
-  return ((size_t)2 * F2 * PLANE + (size_t)2 * Q * TWV + (size_t)F2 * n_ant) * sizeof(float4);
+  return ((size_t)2 * F2 * PLANE + 8 + (size_t)2 * Q * TWV + (size_t)F2 * n_ant) * sizeof(float4);
 }
 
 // ================================================================ tensor-core column pass
@@ -699,23 +742,24 @@ int launch_fused(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
   return EPIC_OK;
 }
 
-// dual-residue kernel (four products, tap gather, one layout): sized for two CTAs per SM
-template <int Q, int NB, bool STG>
+// dual-residue kernel (one layout): sized for two CTAs per SM
+template <int Q, int NPROD, bool DELTA, int NB, bool STG>
 int launch_fused_dual(const epic_plan* p, FusedParams P, cudaStream_t s) {
-  constexpr int NT = 64 * Q;
+  constexpr int NT = 64 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
   P.pairs_per_batch = F2;
-  P.nb = (P.n_t + F2 - 1) / F2;
+  const int per_batch = P.n_pol == 2 ? F2 : 2 * F2;  // time samples per batch
+  P.nb = (P.n_t + per_batch - 1) / per_batch;
   P.total = (long long)P.n_chan * (Q / 2) * P.nb;
   const size_t smem = fused_dual_smem_bytes<Q>(P.n_ant) + (STG ? fused_stage_bytes(P.n_ent) : 0);
-  auto kern = epic_fused_dual_kernel<Q, NB, STG>;
+  auto kern = epic_fused_dual_kernel<Q, NPROD, DELTA, NB, STG>;
   if (smem > 48 * 1024)
     EPIC_CUDA_TRY(cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  // tensor-memory kernels: the occupancy query answers 1; two CTAs (2 x 256 of the 512 columns for Q = 4) share an SM
+  // tensor-memory kernels: the occupancy query answers 1; two CTAs (at most 2 x 256 of the 512 columns) share an SM
   const int per_sm = 2 * (smem + 1024) <= (size_t)227 * 1024 ? 2 : 1;
   const int grid = (int)std::min<long long>(P.total, (long long)per_sm * p->n_sm);
-  if ((size_t)grid * 2 * 2 * 4 * 16 * NT * sizeof(float) > p->scratch_bytes) return EPIC_ERR_RANGE;
+  if ((size_t)grid * 2 * 2 * NACC * 16 * NT * sizeof(float) > p->scratch_bytes) return EPIC_ERR_RANGE;
   kern<<<grid, NT, smem, s>>>(P);
-  epic_fused_dual_fixup<Q><<<(unsigned)(P.total / P.nb), NT, 0, s>>>(P, grid);
+  epic_fused_dual_fixup<Q, NPROD><<<(unsigned)(P.total / P.nb), NT, 0, s>>>(P, grid);
   EPIC_CUDA_TRY(cudaGetLastError());
   return EPIC_OK;
 }
@@ -724,22 +768,15 @@ template <int Q, int NPROD, bool DELTA>
 int launch_fused_nb(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
   // elements y + 16 of a row/column are read only while y < NB (the rest of the block is empty)
   const bool pc = P.cell_stride != 0, nb12 = std::max(p->R, p->Cc) <= 16 + 12;
-  if constexpr (!DELTA && NPROD == 4) {  // two residues per CTA from one gather (needs the scratch for its partial sums)
-    if (!pc && (size_t)2 * p->n_sm * 2 * 2 * 4 * 16 * 64 * Q * sizeof(float) <= p->scratch_bytes) {
-      const bool stg = 2 * (fused_dual_smem_bytes<Q>(P.n_ant) + fused_stage_bytes(P.n_ent) + 1024 + 128) <= (size_t)227 * 1024;
-      if (stg) return nb12 ? launch_fused_dual<Q, 12, true>(p, P, s) : launch_fused_dual<Q, 16, true>(p, P, s);
-      if (2 * (fused_dual_smem_bytes<Q>(P.n_ant) + 1024 + 128) <= (size_t)227 * 1024)
-        return nb12 ? launch_fused_dual<Q, 12, false>(p, P, s) : launch_fused_dual<Q, 16, false>(p, P, s);
-    }
-  }
+  if (pc)  // one layout per channel: the single-residue kernel that reloads its cell records per channel
+    return nb12 ? launch_fused<Q, NPROD, DELTA, 12, true>(p, P, s) : launch_fused<Q, NPROD, DELTA, 16, true>(p, P, s);
+  // one-layout plans: two residues per CTA from one gather (epic_fused_dual_kernel).  Its shared memory is never
+  // more than the single-residue kernel's (same planes, half the voltages), so it fits whenever fused_supported said yes.
   if constexpr (!DELTA) {  // staged gather tables, if two CTAs still fit an SM with them
-    if (!pc && 2 * (fused_smem_bytes<Q>(P.n_ant) + fused_stage_bytes(P.n_ent) + 1024 + 128) <= (size_t)227 * 1024)
-      return nb12 ? launch_fused<Q, NPROD, DELTA, 12, false, true>(p, P, s)
-                  : launch_fused<Q, NPROD, DELTA, 16, false, true>(p, P, s);
+    if (2 * (fused_dual_smem_bytes<Q>(P.n_ant) + fused_stage_bytes(P.n_ent) + 1024 + 128) <= (size_t)227 * 1024)
+      return nb12 ? launch_fused_dual<Q, NPROD, false, 12, true>(p, P, s) : launch_fused_dual<Q, NPROD, false, 16, true>(p, P, s);
   }
-  if (nb12)
-    return pc ? launch_fused<Q, NPROD, DELTA, 12, true>(p, P, s) : launch_fused<Q, NPROD, DELTA, 12, false>(p, P, s);
-  return pc ? launch_fused<Q, NPROD, DELTA, 16, true>(p, P, s) : launch_fused<Q, NPROD, DELTA, 16, false>(p, P, s);
+  return nb12 ? launch_fused_dual<Q, NPROD, DELTA, 12, false>(p, P, s) : launch_fused_dual<Q, NPROD, DELTA, 16, false>(p, P, s);
 }
 
 template <int Q>
@@ -749,7 +786,7 @@ int launch_fused_q(const epic_plan* p, const FusedParams& P, int n_products, cud
   const FusedTables* ft = static_cast<const FusedTables*>(p->d_fused);
   const bool delta = p->t.is_delta != 0 && P.phasor == nullptr && ft->max_cnt <= 16u;
 #ifdef EPIC_FUSED_DEV_ONE  // development builds: compile a single instantiation
-  if (Q == 4 && n_products == 2 && delta) return launch_fused<4, 2, true, 12, false, false>(p, P, s);
+  if (Q == 4 && n_products == 2 && delta) return launch_fused_dual<4, 2, true, 12, false>(p, P, s);
   return EPIC_ERR_RANGE;
 #else
   switch (n_products) {
@@ -892,8 +929,10 @@ int fused_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products) 
   const int Q = p->N / S;
   const int nt = 64 * Q;
   const int a_pad = (p->n_ant + 3) & ~3;  // a short tail group is fetched as bytes (prefetch_batch)
-  if ((long long)F * (a_pad / 4) > (long long)MAXW * nt) return 0;  // prefetch registers
-  const size_t smem = Q == 2 ? fused_smem_bytes<2>(a_pad) : fused_smem_bytes<4>(a_pad);
+  const int ff = p->n_layout > 1 ? F : F2;  // pairs per batch: per-channel plans run the single-residue kernel
+  if ((long long)ff * (a_pad / 4) > (long long)MAXW * nt) return 0;  // prefetch registers
+  const size_t smem = p->n_layout > 1 ? (Q == 2 ? fused_smem_bytes<2>(a_pad) : fused_smem_bytes<4>(a_pad))
+                                      : (Q == 2 ? fused_dual_smem_bytes<2>(a_pad) : fused_dual_smem_bytes<4>(a_pad));
   return smem <= (size_t)200 * 1024 ? 1 : 0;
 }
 
@@ -906,6 +945,7 @@ int tensor_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products)
   if (!p->fused_ok || !fused_supported(p, is_cf32, n_pol, n_products)) return 0;
   const FusedTables* ft = static_cast<const FusedTables*>(p->d_fused);
   if (p->N != TC_N || !ft->a_tab || n_pol != 2 || p->n_layout != 1) return 0;
+  if ((long long)F * (((p->n_ant + 3) & ~3) / 4) > (long long)MAXW * TC_NT) return 0;  // prefetch registers
   return tc_smem_bytes((p->n_ant + 3) & ~3) <= (size_t)226 * 1024 ? 1 : 0;
 }
 
