@@ -271,7 +271,7 @@ __device__ __forceinline__ void col_task_tmem2(const float4* __restrict__ col, c
 }
 
 // partial sums of split units, as epic_fused_fixup, for units of two residues: [cta][slot][residue][4][16][NT]
-template <int Q, int NPROD>
+template <int Q, int NPROD, int NRES>
 __global__ void __launch_bounds__(64 * Q) epic_fused_dual_fixup(FusedParams P, int main_grid) {
   constexpr int NT = 64 * Q, KPT = 16, N = 32 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
   const int unit = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -280,17 +280,17 @@ __global__ void __launch_bounds__(64 * Q) epic_fused_dual_fixup(FusedParams P, i
   if (b_lo == b_hi) return;  // the unit ran in one CTA and was added directly
   const int l1 = (warp & 1) * 16 + (lane >> 1);
   const int rho = (warp >> 1) * 2 + (lane & 1);
-  const int c = unit / (Q / 2), u2 = unit - c * (Q / 2);
+  const int c = unit / (Q / NRES), u2 = unit - c * (Q / NRES);
   const size_t plane = (size_t)N * N;
-  for (int res = 0; res < 2; ++res) {
-    float* o = P.out + (size_t)c * P.n_planes * plane + (Q * l1 + 2 * u2 + res) + (size_t)rho * N;
+  for (int res = 0; res < NRES; ++res) {
+    float* o = P.out + (size_t)c * P.n_planes * plane + (Q * l1 + NRES * u2 + res) + (size_t)rho * N;
     for (int k = 0; k < KPT; ++k) {
       float v[NACC];
 #pragma unroll
       for (int q = 0; q < NACC; ++q) v[q] = 0.0f;
       for (int b = b_lo; b <= b_hi; ++b) {
         const int slot = (first <= P.total * b / G) ? 0 : 1;
-        const float* part = P.partial + ((size_t)((b * 2 + slot) * 2 + res) * NACC * KPT) * NT + tid;
+        const float* part = P.partial + ((size_t)((b * 2 + slot) * NRES + res) * NACC * KPT) * NT + tid;
 #pragma unroll
         for (int q = 0; q < NACC; ++q) v[q] += part[(size_t)(q * KPT + k) * NT];
       }
@@ -299,33 +299,37 @@ __global__ void __launch_bounds__(64 * Q) epic_fused_dual_fixup(FusedParams P, i
   }
 }
 
-template <int Q, int NPROD, bool DELTA, int NB, bool STG>
+// NRES residues per CTA: 2, or all 4 (Q = 4, one or two products: 4 x 32 accumulator columns per thread) with one
+// pair per batch; the work per batch is the same 4 (pair, residue) column tasks per thread either way.
+template <int Q, int NPROD, bool DELTA, int NB, bool STG, int NRES>
 __global__ void __launch_bounds__(64 * Q, 2) epic_fused_dual_kernel(FusedParams P) {
   static_assert(!(STG && DELTA), "staged tables: tap kernels only");
-  constexpr int NT = 64 * Q, N = 32 * Q, HQ = Q / 2, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
+  static_assert(NRES == 2 || (NRES == 4 && Q == 4 && NPROD != 4), "four residues: Q = 4, accumulators of 32 columns");
+  constexpr int NT = 64 * Q, N = 32 * Q, HQ = Q / NRES, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
+  constexpr int FB = 4 / NRES;               // pairs per batch
   constexpr int CPT = NPROD == 4 ? 64 : 32;  // accumulator columns per thread and residue
+  // Residue r's planes start SET cells after residue r-1's: FB planes plus a skew of 8 / NRES cells.  In the row pass
+  // the (h, residue) tasks of a row are adjacent lanes; without the skew the residues' stores of one row fall in the
+  // same 16-byte bank groups (216 M of 445 M store wavefronts were conflicts before it)
+  constexpr int SET = FB * PLANE + 8 / NRES;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  float4* gA = reinterpret_cast<float4*>(smem_raw);  // [F2][32][HS] gridded planes, then residue 0's rows (in place)
-  // residue 1's planes are skewed by 4 cells (64 bytes): in the row pass the (h, residue) tasks of two rows make a
-  // quarter-warp, and without the skew the two residues' stores of one row fall in the same 16-byte bank groups
-  // (216 M of 445 M store wavefronts were conflicts before)
-  float4* gB = gA + F2 * PLANE + 4;                  // [F2][32][HS] residue 1's rows
-  float4* tws = gA + 2 * F2 * PLANE + 8;             // [2Q][TWV]
-  float4* E = tws + 2 * Q * TWV;                     // [F2][A]
+  float4* gA = reinterpret_cast<float4*>(smem_raw);  // [NRES] x [FB][32][HS]: set 0 holds the gridded planes, then residue 0's rows (in place)
+  float4* tws = gA + NRES * SET;                     // [2Q][TWV]
+  float4* E = tws + 2 * Q * TWV;                     // [FB][A]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
   const long long g0 = P.total * (long long)blockIdx.x / gridDim.x;
   const long long g1 = P.total * (long long)(blockIdx.x + 1) / gridDim.x;
   if (g0 >= g1) return;
-  constexpr int TCOLS1 = (Q == 4 ? 2 : 1) * CPT, TCOLS = 2 * TCOLS1;  // one block of accumulator columns per residue
+  constexpr int TCOLS1 = (Q == 4 ? 2 : 1) * CPT, TCOLS = NRES * TCOLS1;  // one block of accumulator columns per residue
 
-  int unit = (int)(g0 / P.nb);  // unit = (channel, residue pair)
+  int unit = (int)(g0 / P.nb);  // unit = (channel, group of NRES residues)
   uint2 info[S * S / NT];
 #pragma unroll
   for (int j = 0; j < S * S / NT; ++j) info[j] = __ldg(P.cell_info + tid + j * NT);
-  for (int i = tid; i < 2 * F2 * PLANE + 8; i += NT) gA[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);  // rows >= R stay zero
+  for (int i = tid; i < NRES * SET; i += NT) gA[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);  // rows >= R stay zero
   for (int i = tid; i < 2 * Q * TWV; i += NT) tws[i] = __ldg(P.tw + i);
-  float2* tap_s = reinterpret_cast<float2*>(E + F2 * P.n_ant);
+  float2* tap_s = reinterpret_cast<float2*>(E + FB * P.n_ant);
   uint16_t* ant_s = reinterpret_cast<uint16_t*>(tap_s + P.n_ent);
   if constexpr (STG) {
     for (int i = tid; i < P.n_ent; i += NT) { tap_s[i] = __ldg(P.ent_tap + i); ant_s[i] = __ldg(P.ent_ant + i); }
@@ -342,7 +346,7 @@ __global__ void __launch_bounds__(64 * Q, 2) epic_fused_dual_kernel(FusedParams 
 #pragma unroll
     for (int i = 0; i < 16; ++i) zero[i] = 0.0f;
 #pragma unroll
-    for (int res = 0; res < 2; ++res)
+    for (int res = 0; res < NRES; ++res)
 #pragma unroll
       for (int c = 0; c < CPT / 16; ++c) tmem_st16(taddr + res * TCOLS1 + 16 * c, zero);
     tmem_wait_st();
@@ -354,9 +358,9 @@ __global__ void __launch_bounds__(64 * Q, 2) epic_fused_dual_kernel(FusedParams 
     const int c = unit / HQ, u2 = unit - c * HQ;
     const size_t plane = (size_t)N * N;
 #pragma unroll 1
-    for (int res = 0; res < 2; ++res) {
-      float* o = P.out + (size_t)c * P.n_planes * plane + (Q * l1 + 2 * u2 + res);
-      float* part = P.partial + ((size_t)((blockIdx.x * 2 + slot) * 2 + res) * NACC * 16) * NT + tid;
+    for (int res = 0; res < NRES; ++res) {
+      float* o = P.out + (size_t)c * P.n_planes * plane + (Q * l1 + NRES * u2 + res);
+      float* part = P.partial + ((size_t)((blockIdx.x * 2 + slot) * NRES + res) * NACC * 16) * NT + tid;
       const uint32_t ta = taddr + res * TCOLS1;
       constexpr int PPC = NPROD == 4 ? 4 : 8;  // pixels per 16-column chunk
 #pragma unroll
@@ -393,42 +397,42 @@ __global__ void __launch_bounds__(64 * Q, 2) epic_fused_dual_kernel(FusedParams 
   const int first_unit = unit;
   int seg_begin = b;
   PrefetchSlots ps;
-  prefetch_init<NT, F2>(P, tid, ps);
+  prefetch_init<NT, FB>(P, tid, ps);
   uint32_t wlo[MAXW], whi[MAXW];
-  prefetch_batch<NT, F2>(P, ps, unit / HQ, b, wlo, whi);
+  prefetch_batch<NT, FB>(P, ps, unit / HQ, b, wlo, whi);
   unpack_batch<DELTA>(P, ps, E, wlo, whi, unit / HQ);
   __syncthreads();
 
-  const int ntask = F2 * P.R * 4;  // (pair, row, h, residue), residue fastest: a row's four tasks are adjacent lanes
+  const int ntask = FB * P.R * 2 * NRES;  // (pair, row, h, residue), residue fastest: a row's tasks are adjacent lanes of one warp
   for (long long g = g0; g < g1; ++g) {
     int unit_n = unit, b_n = b + 1;
     if (b_n == P.nb) { b_n = 0; ++unit_n; }
     const bool more = g + 1 < g1;
-    if (more) prefetch_batch<NT, F2>(P, ps, unit_n / HQ, b_n, wlo, whi);
+    if (more) prefetch_batch<NT, FB>(P, ps, unit_n / HQ, b_n, wlo, whi);
 
-    gather_batch<NT, DELTA, STG, DELTA, F2>(P, E, gA, info, ant_s, tap_s);
+    gather_batch<NT, DELTA, STG, DELTA, FB>(P, E, gA, info, ant_s, tap_s);
     __syncthreads();
 
-    const int l2a = 2 * (unit % HQ);
+    const int l2a = NRES * (unit % HQ);
     for (int base = warp * 32; base < ntask; base += NT) {
       const int task = base + lane;
       const bool valid = task < ntask;
       // idle lanes transform the all-zero row 31 of plane 0 (they exist only when R < 32)
       int f = 0, y = S - 1, h = 0, res = 0;
-      if (valid) { res = task & 1; h = (task >> 1) & 1; const int p = task >> 2; f = p / P.R; y = p - f * P.R; }
+      if (valid) { res = task % NRES; h = (task / NRES) & 1; const int p = task / (2 * NRES); f = p / P.R; y = p - f * P.R; }
       const float4* src = gA + f * PLANE + y * HS;
-      row_task_dual<NB>(src, (res ? gB : gA) + f * PLANE + y * HS, tws + (l2a + res + Q * h) * TWV, h, valid);
+      row_task_dual<NB>(src, gA + res * SET + f * PLANE + y * HS, tws + (l2a + res + Q * h) * TWV, h, valid);
     }
     __syncthreads();
 
     if (more) unpack_batch<DELTA>(P, ps, E, wlo, whi, unit_n / HQ);  // E was last read by this batch's gather
 #pragma unroll 1
-    for (int rf = 0; rf < 2 * F2; ++rf) {
-      const int res = rf / F2, f = rf - res * F2;
+    for (int rf = 0; rf < NRES * FB; ++rf) {
+      const int res = rf / FB, f = rf - res * FB;
       int tw_off = rho * TWV;
       asm volatile("" : "+r"(tw_off));
-      if constexpr (NPROD == 4) col_task_tmem<NB>((res ? gB : gA) + f * PLANE + l1, tws + tw_off, taddr + res * TCOLS1);
-      else col_task_tmem2<NB>((res ? gB : gA) + f * PLANE + l1, tws + tw_off, taddr + res * TCOLS1);
+      if constexpr (NPROD == 4) col_task_tmem<NB>(gA + res * SET + f * PLANE + l1, tws + tw_off, taddr + res * TCOLS1);
+      else col_task_tmem2<NB>(gA + res * SET + f * PLANE + l1, tws + tw_off, taddr + res * TCOLS1);
     }
 
     if (unit_n != unit || !more) {
@@ -442,8 +446,9 @@ __global__ void __launch_bounds__(64 * Q, 2) epic_fused_dual_kernel(FusedParams 
 }
 
 template <int Q>
-size_t fused_dual_smem_bytes(int n_ant) {
-  return ((size_t)2 * F2 * PLANE + 8 + (size_t)2 * Q * TWV + (size_t)F2 * n_ant) * sizeof(float4);
+size_t fused_dual_smem_bytes(int n_ant, int nres = 2) {
+  const int fb = 4 / nres;
+  return ((size_t)nres * (fb * PLANE + 8 / nres) + (size_t)2 * Q * TWV + (size_t)fb * n_ant) * sizeof(float4);
 }
 
 // ================================================================ tensor-core column pass
@@ -743,23 +748,23 @@ int launch_fused(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
 }
 
 // dual-residue kernel (one layout): sized for two CTAs per SM
-template <int Q, int NPROD, bool DELTA, int NB, bool STG>
+template <int Q, int NPROD, bool DELTA, int NB, bool STG, int NRES = 2>
 int launch_fused_dual(const epic_plan* p, FusedParams P, cudaStream_t s) {
-  constexpr int NT = 64 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
-  P.pairs_per_batch = F2;
-  const int per_batch = P.n_pol == 2 ? F2 : 2 * F2;  // time samples per batch
+  constexpr int NT = 64 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1), FB = 4 / NRES;
+  P.pairs_per_batch = FB;
+  const int per_batch = P.n_pol == 2 ? FB : 2 * FB;  // time samples per batch
   P.nb = (P.n_t + per_batch - 1) / per_batch;
-  P.total = (long long)P.n_chan * (Q / 2) * P.nb;
-  const size_t smem = fused_dual_smem_bytes<Q>(P.n_ant) + (STG ? fused_stage_bytes(P.n_ent) : 0);
-  auto kern = epic_fused_dual_kernel<Q, NPROD, DELTA, NB, STG>;
+  P.total = (long long)P.n_chan * (Q / NRES) * P.nb;
+  const size_t smem = fused_dual_smem_bytes<Q>(P.n_ant, NRES) + (STG ? fused_stage_bytes(P.n_ent) : 0);
+  auto kern = epic_fused_dual_kernel<Q, NPROD, DELTA, NB, STG, NRES>;
   if (smem > 48 * 1024)
     EPIC_CUDA_TRY(cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   // tensor-memory kernels: the occupancy query answers 1; two CTAs (at most 2 x 256 of the 512 columns) share an SM
   const int per_sm = 2 * (smem + 1024) <= (size_t)227 * 1024 ? 2 : 1;
   const int grid = (int)std::min<long long>(P.total, (long long)per_sm * p->n_sm);
-  if ((size_t)grid * 2 * 2 * NACC * 16 * NT * sizeof(float) > p->scratch_bytes) return EPIC_ERR_RANGE;
+  if ((size_t)grid * 2 * NRES * NACC * 16 * NT * sizeof(float) > p->scratch_bytes) return EPIC_ERR_RANGE;
   kern<<<grid, NT, smem, s>>>(P);
-  epic_fused_dual_fixup<Q, NPROD><<<(unsigned)(P.total / P.nb), NT, 0, s>>>(P, grid);
+  epic_fused_dual_fixup<Q, NPROD, NRES><<<(unsigned)(P.total / P.nb), NT, 0, s>>>(P, grid);
   EPIC_CUDA_TRY(cudaGetLastError());
   return EPIC_OK;
 }
@@ -770,13 +775,16 @@ int launch_fused_nb(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
   const bool pc = P.cell_stride != 0, nb12 = std::max(p->R, p->Cc) <= 16 + 12;
   if (pc)  // one layout per channel: the single-residue kernel that reloads its cell records per channel
     return nb12 ? launch_fused<Q, NPROD, DELTA, 12, true>(p, P, s) : launch_fused<Q, NPROD, DELTA, 16, true>(p, P, s);
-  // one-layout plans: two residues per CTA from one gather (epic_fused_dual_kernel).  Its shared memory is never
-  // more than the single-residue kernel's (same planes, half the voltages), so it fits whenever fused_supported said yes.
+  // one-layout plans: NR residues per CTA from one gather (epic_fused_dual_kernel): all four of a channel when the
+  // accumulators are 32 columns per residue (Q = 4, one or two products; C2 32.3 -> 33.5 M frames/s over two), else
+  // two.  Its shared memory is never more than the single-residue kernel's (same planes, fewer voltages), so it fits
+  // whenever fused_supported said yes.
+  constexpr int NR = (Q == 4 && NPROD != 4) ? 4 : 2;
   if constexpr (!DELTA) {  // staged gather tables, if two CTAs still fit an SM with them
-    if (2 * (fused_dual_smem_bytes<Q>(P.n_ant) + fused_stage_bytes(P.n_ent) + 1024 + 128) <= (size_t)227 * 1024)
-      return nb12 ? launch_fused_dual<Q, NPROD, false, 12, true>(p, P, s) : launch_fused_dual<Q, NPROD, false, 16, true>(p, P, s);
+    if (2 * (fused_dual_smem_bytes<Q>(P.n_ant, NR) + fused_stage_bytes(P.n_ent) + 1024 + 128) <= (size_t)227 * 1024)
+      return nb12 ? launch_fused_dual<Q, NPROD, false, 12, true, NR>(p, P, s) : launch_fused_dual<Q, NPROD, false, 16, true, NR>(p, P, s);
   }
-  return nb12 ? launch_fused_dual<Q, NPROD, DELTA, 12, false>(p, P, s) : launch_fused_dual<Q, NPROD, DELTA, 16, false>(p, P, s);
+  return nb12 ? launch_fused_dual<Q, NPROD, DELTA, 12, false, NR>(p, P, s) : launch_fused_dual<Q, NPROD, DELTA, 16, false, NR>(p, P, s);
 }
 
 template <int Q>
@@ -786,7 +794,7 @@ int launch_fused_q(const epic_plan* p, const FusedParams& P, int n_products, cud
   const FusedTables* ft = static_cast<const FusedTables*>(p->d_fused);
   const bool delta = p->t.is_delta != 0 && P.phasor == nullptr && ft->max_cnt <= 16u;
 #ifdef EPIC_FUSED_DEV_ONE  // development builds: compile a single instantiation
-  if (Q == 4 && n_products == 2 && delta) return launch_fused_dual<4, 2, true, 12, false>(p, P, s);
+  if (Q == 4 && n_products == 2 && delta) return launch_fused_dual<4, 2, true, 12, false, 4>(p, P, s);
   return EPIC_ERR_RANGE;
 #else
   switch (n_products) {
@@ -929,7 +937,7 @@ int fused_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products) 
   const int Q = p->N / S;
   const int nt = 64 * Q;
   const int a_pad = (p->n_ant + 3) & ~3;  // a short tail group is fetched as bytes (prefetch_batch)
-  const int ff = p->n_layout > 1 ? F : F2;  // pairs per batch: per-channel plans run the single-residue kernel
+  const int ff = p->n_layout > 1 ? F : F2;  // pairs per batch (at most): per-channel plans run the single-residue kernel
   if ((long long)ff * (a_pad / 4) > (long long)MAXW * nt) return 0;  // prefetch registers
   const size_t smem = p->n_layout > 1 ? (Q == 2 ? fused_smem_bytes<2>(a_pad) : fused_smem_bytes<4>(a_pad))
                                       : (Q == 2 ? fused_dual_smem_bytes<2>(a_pad) : fused_dual_smem_bytes<4>(a_pad));
