@@ -426,7 +426,7 @@ def run_epic(args, wl):
     # the previous chunk's kernels (compute stream), and the accumulated images are copied back.  The call is
     # synchronous and runs on the library's own streams, so this leg is timed with the host clock around the call,
     # the device idle on both sides.
-    n_chunks = max(1, min(args.e2e_chunks, wl.n_t))
+    n_chunks = max(0, min(args.e2e_chunks, wl.n_t))
 
     class _HostTimed:
         def __init__(self, ms):
@@ -498,7 +498,7 @@ def run_epic(args, wl):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(volt.nbytes),
                 "d2h_bytes_per_step": int(out.numel() * 4), "measured": not args.no_e2e,
                 "how": f"one epic_image_host call (C ABI, HOST pointers: pinned voltages in, pinned out_accum out) per step: inside "
-                       f"the library {n_chunks} time chunks (the first half as long as the others), H2D of chunk k+1 on a copy "
+                       f"the library {n_chunks if n_chunks else 'an automatic number of'} time chunks (the first half as long as the others), H2D of chunk k+1 on a copy "
                        f"stream overlapped with the kernels of chunk k, one D2H of the accumulated images; synchronous call "
                        f"timed with the host clock, device idle before and after"},
         "gpu_launches": int(launches),
@@ -573,7 +573,7 @@ def main():
                     help="skip the other_configs block (C3, C4, C5, streamed, tensor, wide) of the default C2 run")
     ap.add_argument("--input-order", default="tcpa", choices=["tcpa", "tcap"], help="tcap = [T][C][A][Np], transposed in the load")
     ap.add_argument("--delay-phasors", action="store_true", help="apply per-(channel, pol, antenna) delay phasors")
-    ap.add_argument("--e2e-chunks", type=int, default=4, help="time chunks of the end-to-end leg (H2D overlapped)")
+    ap.add_argument("--e2e-chunks", type=int, default=0, help="time chunks of the end-to-end leg (H2D overlapped); 0 = the library's choice")
     ap.add_argument("--scratch-mib", type=int, default=0, help="cap the per-batch scratch (tiled / two-pass paths)")
     ap.add_argument("--per-channel-cells", action="store_true",
                     help="configs 2-4 with one antenna layout per 25 kHz channel (cell = lambda_c/2) and, for 3 and 4, "

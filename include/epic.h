@@ -133,7 +133,8 @@ EPIC_API int epic_image(epic_plan* plan, const void* voltages, int n_t, int n_ch
 
 /* The same gulp from HOST memory, end to end: voltages_host HOST uint8 (layout as in epic_image; pinned memory makes the
  * copies asynchronous, pageable memory works), out_accum_host HOST float[n_chan][planes][N][N].  The library cuts the gulp
- * into n_chunks time chunks (<= 0: 4; the first one half as long, its copy is the one nothing hides), copies chunk k+1
+ * into n_chunks time chunks (<= 0: chosen from the gulp's size, 1..8; the first one half as long, its copy is the one
+ * nothing hides), copies chunk k+1
  * host->device on its own stream while epic_image of chunk k runs (double-buffered device staging owned by the plan),
  * and copies the accumulated images back.  accumulate != 0: the images are ADDED to the contents of out_accum_host (which
  * is copied to the device first); accumulate == 0: out_accum_host is overwritten.  SYNCHRONOUS: returns when

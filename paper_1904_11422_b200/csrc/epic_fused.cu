@@ -273,8 +273,12 @@ __device__ __forceinline__ void col_task_tmem2(const float4* __restrict__ col, c
 // partial sums of split units, as epic_fused_fixup, for units of two residues: [cta][slot][residue][4][16][NT]
 template <int Q, int NPROD, int NRES>
 __global__ void __launch_bounds__(64 * Q) epic_fused_dual_fixup(FusedParams P, int main_grid) {
+  // one CTA per (unit, residue): with NRES = 4 a unit is a whole channel and every unit is split between CTAs of the
+  // main kernel, so this kernel touches every pixel; (unit, residue) CTAs give it 4x the parallelism of one CTA per
+  // unit (measured 0.19 -> see profiles/r02_fused_c2_c3_ncu.md)
   constexpr int NT = 64 * Q, KPT = 16, N = 32 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
-  const int unit = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int unit = blockIdx.x / NRES, res = blockIdx.x - unit * NRES;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const long long G = main_grid, first = (long long)unit * P.nb, last = first + P.nb - 1;
   const int b_lo = (int)(((first + 1) * G - 1) / P.total), b_hi = (int)(((last + 1) * G - 1) / P.total);
   if (b_lo == b_hi) return;  // the unit ran in one CTA and was added directly
@@ -282,21 +286,22 @@ __global__ void __launch_bounds__(64 * Q) epic_fused_dual_fixup(FusedParams P, i
   const int rho = (warp >> 1) * 2 + (lane & 1);
   const int c = unit / (Q / NRES), u2 = unit - c * (Q / NRES);
   const size_t plane = (size_t)N * N;
-  for (int res = 0; res < NRES; ++res) {
-    float* o = P.out + (size_t)c * P.n_planes * plane + (Q * l1 + NRES * u2 + res) + (size_t)rho * N;
-    for (int k = 0; k < KPT; ++k) {
-      float v[NACC];
+  float* o = P.out + (size_t)c * P.n_planes * plane + (Q * l1 + NRES * u2 + res) + (size_t)rho * N;
+  float v[KPT][NACC];
 #pragma unroll
-      for (int q = 0; q < NACC; ++q) v[q] = 0.0f;
-      for (int b = b_lo; b <= b_hi; ++b) {
-        const int slot = (first <= P.total * b / G) ? 0 : 1;
-        const float* part = P.partial + ((size_t)((b * 2 + slot) * NRES + res) * NACC * KPT) * NT + tid;
+  for (int k = 0; k < KPT; ++k)
 #pragma unroll
-        for (int q = 0; q < NACC; ++q) v[q] += part[(size_t)(q * KPT + k) * NT];
-      }
-      add_pixel<NPROD>(o + (size_t)k * 2 * Q * N, plane, v);
-    }
+    for (int q = 0; q < NACC; ++q) v[k][q] = 0.0f;
+  for (int b = b_lo; b <= b_hi; ++b) {  // in CTA order: the sum does not depend on scheduling
+    const int slot = (first <= P.total * b / G) ? 0 : 1;  // does the segment start the CTA's range?
+    const float* part = P.partial + ((size_t)((b * 2 + slot) * NRES + res) * NACC * KPT) * NT + tid;
+#pragma unroll
+    for (int k = 0; k < KPT; ++k)
+#pragma unroll
+      for (int q = 0; q < NACC; ++q) v[k][q] += __ldcs(part + (size_t)(q * KPT + k) * NT);
   }
+#pragma unroll
+  for (int k = 0; k < KPT; ++k) add_pixel<NPROD>(o + (size_t)k * 2 * Q * N, plane, v[k]);
 }
 
 // NRES residues per CTA: 2, or all 4 (Q = 4, one or two products: 4 x 32 accumulator columns per thread) with one
@@ -764,7 +769,7 @@ int launch_fused_dual(const epic_plan* p, FusedParams P, cudaStream_t s) {
   const int grid = (int)std::min<long long>(P.total, (long long)per_sm * p->n_sm);
   if ((size_t)grid * 2 * NRES * NACC * 16 * NT * sizeof(float) > p->scratch_bytes) return EPIC_ERR_RANGE;
   kern<<<grid, NT, smem, s>>>(P);
-  epic_fused_dual_fixup<Q, NPROD, NRES><<<(unsigned)(P.total / P.nb), NT, 0, s>>>(P, grid);
+  epic_fused_dual_fixup<Q, NPROD, NRES><<<(unsigned)(P.total / P.nb) * NRES, NT, 0, s>>>(P, grid);
   EPIC_CUDA_TRY(cudaGetLastError());
   return EPIC_OK;
 }

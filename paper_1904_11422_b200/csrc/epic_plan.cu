@@ -595,7 +595,9 @@ int epic_image_host(epic_plan* plan, const void* voltages_host, int n_t, int n_c
   if (!out_accum_host || (n_t > 0 && !voltages_host)) return EPIC_ERR_ARG;
   const size_t sample_bytes = (size_t)n_chan * n_pol * plan->n_ant;  // one time sample of all channels
   const size_t out_bytes = (size_t)n_chan * n_planes * plan->N * plan->N * sizeof(float);
-  if (n_chunks <= 0) n_chunks = 4;
+  // automatic chunk count: the first chunk's copy is exposed (~ bytes / (2 n) at ~50 GB/s) and every chunk costs a
+  // call (~0.1 ms of launches, flush and fix-up), so n ~ sqrt(bytes / 8 MB): C2 (65.5 MB) 2, C3 (164 MB) 4 (measured on C2: 2 chunks 27.7, 3 27.2, 4 26.8, 6 25.4 M frames/s)
+  if (n_chunks <= 0) n_chunks = std::max(1, std::min(8, (int)std::sqrt((double)n_t * (double)sample_bytes / 8.0e6)));
   n_chunks = std::max(1, std::min(n_chunks, n_t));
   // chunk edges: a short first chunk (its copy is the one nothing can hide), the rest equal
   std::vector<int> edge(1, 0);
