@@ -49,7 +49,8 @@ typedef enum epic_status {
   EPIC_ERR_ARG = -1,   /* NULL pointer, bad shape, even kernel_k, N not a power of two in 8..512 */
   EPIC_ERR_RANGE = -2, /* n_pol not in {1,2}, n_products incompatible with n_pol, n_ant too large */
   EPIC_ERR_CUDA = -3,  /* a CUDA runtime call failed; see epic_last_cuda_error() */
-  EPIC_ERR_NOMEM = -4  /* host or device allocation failed */
+  EPIC_ERR_NOMEM = -4, /* host or device allocation failed */
+  EPIC_ERR_SCRATCH = -5 /* epic_image_noalloc: the call needs more than the library's static scratch array holds */
 } epic_status;
 
 /* Which kernel family epic_image uses.  AUTO picks the fastest one that supports the plan. */
@@ -142,6 +143,26 @@ EPIC_API int epic_image(epic_plan* plan, const void* voltages, int n_t, int n_ch
  * This is the call bench.py's `e2e` leg times. */
 EPIC_API int epic_image_host(epic_plan* plan, const void* voltages_host, int n_t, int n_chan, int n_pol,
                     float* out_accum_host, int accumulate, int n_chunks);
+
+/* epic_image for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc).  Same arguments, semantics and result as epic_image (S1..S6; ADDS into
+ * out_accum; asynchronous on `stream`), for plans the fused kernel of epic_fused.cu takes with ONE layout: N = 64 or
+ * 128, occupied cells within 32 x 32, 4+4-bit voltages (EPIC_ERR_RANGE otherwise; epic_plan_set_path is ignored).
+ * The kernel's scratch -- the partial sums of work units whose time range is split between CTAs -- is not the plan's
+ * cudaMalloc'ed buffer but a file-scope `static __device__` array of epic_noalloc_scratch_bytes() = 80 MiB inside the
+ * library: every GPU that loads libepic.so holds those 80 MiB until the process exits.  The call itself calls no
+ * cudaMalloc, cudaFree or allocating library routine and does not synchronise.  A launch that would need more than
+ * the array holds (256 KiB per resident CTA at N = 128: 74 MiB on a 148-SM B200 with two CTAs per SM, more on a larger GPU)
+ * is refused with EPIC_ERR_SCRATCH before anything is enqueued.  Nothing in the array has to start at zero (every
+ * slot that is read was written by the same call).  ALL calls in the process on one GPU share the array: calls that
+ * overlap on the GPU (different streams, or different plans on different streams) race on it -- issue them on one
+ * stream or order them with events.  The first call on each device looks the array's device address up
+ * (cudaGetSymbolAddress, no allocation); callers that capture graphs make one call outside capture first (n_t = 0 will
+ * do). */
+EPIC_API int epic_image_noalloc(epic_plan* plan, const void* voltages, int n_t, int n_chan, int n_pol,
+                       float* out_accum, epic_stream stream);
+/* Size in bytes of the static scratch array of epic_image_noalloc. */
+EPIC_API long long epic_noalloc_scratch_bytes(void);
 
 /* Same with complex fp32 voltages: DEVICE float[n_t][n_chan][n_pol][n_ant][2] (re, im). */
 EPIC_API int epic_image_cf32(epic_plan* plan, const void* voltages_cf32, int n_t, int n_chan, int n_pol,

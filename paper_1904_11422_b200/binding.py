@@ -14,7 +14,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libepic.so")
 
 EPIC_OK = 0
-EPIC_ERR_ARG, EPIC_ERR_RANGE, EPIC_ERR_CUDA, EPIC_ERR_NOMEM = -1, -2, -3, -4
+EPIC_ERR_ARG, EPIC_ERR_RANGE, EPIC_ERR_CUDA, EPIC_ERR_NOMEM, EPIC_ERR_SCRATCH = -1, -2, -3, -4, -5
 EPIC_PATH_AUTO, EPIC_PATH_TWOPASS, EPIC_PATH_FUSED, EPIC_PATH_TILED, EPIC_PATH_TENSOR, EPIC_PATH_STREAM = 0, 1, 2, 3, 4, 5
 EPIC_ORDER_TCPA, EPIC_ORDER_TCAP = 0, 1
 
@@ -33,6 +33,8 @@ SYMBOLS = {
     "epic_image": (_i, [_vp, _vp, _i, _i, _i, _vp, _vp]),
     "epic_image_cf32": (_i, [_vp, _vp, _i, _i, _i, _vp, _vp]),
     "epic_image_host": (_i, [_vp, _vp, _i, _i, _i, _vp, _i, _i]),
+    "epic_image_noalloc": (_i, [_vp, _vp, _i, _i, _i, _vp, _vp]),
+    "epic_noalloc_scratch_bytes": (ctypes.c_longlong, []),
     "epic_autocorr_remove": (_i, [_vp, _vp, _i, _i, _i, _vp, _vp]),
     "epic_plan_get_n": (_i, [_vp]),
     "epic_plan_get_n_planes": (_i, [_vp, _i]),
@@ -241,6 +243,14 @@ class Plan:
         _check(lib().epic_image(self._h, _ptr(voltages), n_t, n_chan, n_pol, _ptr(out_accum),
                                 _stream(stream)), "epic_image")
 
+    def image_noalloc(self, voltages, n_t: int, n_chan: int, n_pol: int, out_accum, stream=None) -> None:
+        """epic_image_noalloc: epic_image for callers that must not allocate -- the fused kernel with its scratch in
+        the library's static 80 MiB device array (one-layout plans with N = 64 / 128 and a 32 x 32 support); calls that
+        overlap on the GPU race on that array."""
+        self._check_call(voltages, "uint8", 1, n_t, n_chan, n_pol, out_accum)
+        _check(lib().epic_image_noalloc(self._h, _ptr(voltages), n_t, n_chan, n_pol, _ptr(out_accum),
+                                        _stream(stream)), "epic_image_noalloc")
+
     def image_host(self, voltages_host, n_t: int, n_chan: int, n_pol: int, out_accum_host, accumulate: bool = True,
                    n_chunks: int = 0) -> None:
         """epic_image_host: the same gulp from HOST memory (numpy arrays or CPU torch tensors, pinned or not): the
@@ -298,6 +308,14 @@ def epic_plan_destroy(plan: Optional[Plan]) -> None:
 
 def epic_image(plan: Plan, voltages, n_t, n_chan, n_pol, out_accum, stream=None) -> None:
     plan.image(voltages, n_t, n_chan, n_pol, out_accum, stream)
+
+
+def epic_image_noalloc(plan: Plan, voltages, n_t, n_chan, n_pol, out_accum, stream=None) -> None:
+    plan.image_noalloc(voltages, n_t, n_chan, n_pol, out_accum, stream)
+
+
+def epic_noalloc_scratch_bytes() -> int:
+    return int(lib().epic_noalloc_scratch_bytes())
 
 
 def epic_image_host(plan: Plan, voltages_host, n_t, n_chan, n_pol, out_accum_host, accumulate=True, n_chunks=0) -> None:

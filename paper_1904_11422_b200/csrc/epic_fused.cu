@@ -50,6 +50,16 @@
 #include "epic_packed.cuh"
 #include "epic_fused_core.cuh"
 
+#include <mutex>
+
+// Scratch of epic_image_noalloc (include/epic.h): the partial sums of split work units of the residue-group kernel,
+// in a file-scope static device array instead of the plan's cudaMalloc'ed buffer.  80 MiB: 2 slots x (residues x
+// products = 8) x 16 pixels x 256 threads x 4 B = 256 KiB per resident CTA, x 296 CTAs = 74 MiB on a 148-SM B200.  Every GPU that loads
+// the library holds it until the process exits.  In HOST code this name is a host-side stand-in, not a device
+// address: the address the kernels get comes from cudaGetSymbolAddress (noalloc_scratch_ptr below).
+constexpr size_t EPIC_NOALLOC_SCRATCH_BYTES = (size_t)80 << 20;
+static __device__ __align__(256) unsigned char epic_noalloc_scratch[EPIC_NOALLOC_SCRATCH_BYTES];
+
 namespace epic {
 namespace {
 
@@ -1039,6 +1049,104 @@ int fused_image(epic_plan* p, const ImageArgs& a) {
   else st = launch_fused_q<4>(p, P, a.n_products, a.stream);
   if (st != EPIC_OK) return st;
   p->last_launches = 2;  // the fused kernel and the (tiny) fix-up of split units
+  return EPIC_OK;
+}
+
+// ---------------------------------------------------------------- epic_image_noalloc (include/epic.h)
+namespace {
+
+// Device address of epic_noalloc_scratch on the CURRENT device, looked up once per device (set-up; no allocation).
+constexpr int NOALLOC_MAX_DEVICES = 64;
+void* g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {nullptr};
+std::mutex g_noalloc_mutex;
+
+int noalloc_scratch_ptr(float** out) {
+  int dev = -1;
+  EPIC_CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return EPIC_ERR_RANGE;
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_ptr[dev]) {
+    void* q = nullptr;
+    EPIC_CUDA_TRY(cudaGetSymbolAddress(&q, epic_noalloc_scratch));  // this device's copy of the array
+    if (!q) return EPIC_ERR_CUDA;
+    g_noalloc_ptr[dev] = q;
+  }
+  *out = static_cast<float*>(g_noalloc_ptr[dev]);
+  return EPIC_OK;
+}
+
+// launch_fused_dual with the static array as the partial-sum scratch: same kernels, same launch configuration, so the
+// images are bit-identical to epic_image's.  Nothing in the scratch has to start at zero: the fix-up kernel reads
+// exactly the slots the main kernel of the same call wrote (the segments of the units that were split).
+template <int Q, int NPROD, bool DELTA, int NB, bool STG, int NRES>
+int launch_dual_static(const epic_plan* p, FusedParams P, float* scratch, cudaStream_t s) {
+  constexpr int NT = 64 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1), FB = 4 / NRES;
+  P.partial = scratch;
+  P.pairs_per_batch = FB;
+  const int per_batch = P.n_pol == 2 ? FB : 2 * FB;  // time samples per batch
+  P.nb = (P.n_t + per_batch - 1) / per_batch;
+  P.total = (long long)P.n_chan * (Q / NRES) * P.nb;
+  const size_t smem = fused_dual_smem_bytes<Q>(P.n_ant, NRES) + (STG ? fused_stage_bytes(P.n_ent) : 0);
+  auto kern = epic_fused_dual_kernel<Q, NPROD, DELTA, NB, STG, NRES>;
+  if (smem > 48 * 1024)
+    EPIC_CUDA_TRY(cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int per_sm = 2 * (smem + 1024) <= (size_t)227 * 1024 ? 2 : 1;
+  const int grid = (int)std::min<long long>(P.total, (long long)per_sm * p->n_sm);
+  if ((size_t)grid * 2 * NRES * NACC * 16 * NT * sizeof(float) > EPIC_NOALLOC_SCRATCH_BYTES) return EPIC_ERR_SCRATCH;
+  kern<<<grid, NT, smem, s>>>(P);
+  epic_fused_dual_fixup<Q, NPROD, NRES><<<(unsigned)(P.total / P.nb) * NRES, NT, 0, s>>>(P, grid);
+  EPIC_CUDA_TRY(cudaGetLastError());
+  return EPIC_OK;
+}
+
+// the choices of launch_fused_nb for one-layout plans
+template <int Q, int NPROD, bool DELTA>
+int launch_static_nb(const epic_plan* p, const FusedParams& P, float* scratch, cudaStream_t s) {
+  const bool nb12 = std::max(p->R, p->Cc) <= 16 + 12;
+  constexpr int NR = (Q == 4 && NPROD != 4) ? 4 : 2;
+  if constexpr (!DELTA) {
+    if (2 * (fused_dual_smem_bytes<Q>(P.n_ant, NR) + fused_stage_bytes(P.n_ent) + 1024 + 128) <= (size_t)227 * 1024)
+      return nb12 ? launch_dual_static<Q, NPROD, false, 12, true, NR>(p, P, scratch, s)
+                  : launch_dual_static<Q, NPROD, false, 16, true, NR>(p, P, scratch, s);
+  }
+  return nb12 ? launch_dual_static<Q, NPROD, DELTA, 12, false, NR>(p, P, scratch, s)
+              : launch_dual_static<Q, NPROD, DELTA, 16, false, NR>(p, P, scratch, s);
+}
+
+// the choices of launch_fused_q
+template <int Q>
+int launch_static_q(const epic_plan* p, const FusedParams& P, int n_products, float* scratch, cudaStream_t s) {
+  const FusedTables* ft = static_cast<const FusedTables*>(p->d_fused);
+  const bool delta = p->t.is_delta != 0 && P.phasor == nullptr && ft->max_cnt <= 16u;
+#ifdef EPIC_FUSED_DEV_ONE  // development builds: compile a single instantiation
+  if (Q == 4 && n_products == 2 && delta) return launch_dual_static<4, 2, true, 12, false, 4>(p, P, scratch, s);
+  return EPIC_ERR_RANGE;
+#else
+  switch (n_products) {
+    case 1: return delta ? launch_static_nb<Q, 1, true>(p, P, scratch, s) : launch_static_nb<Q, 1, false>(p, P, scratch, s);
+    case 2: return delta ? launch_static_nb<Q, 2, true>(p, P, scratch, s) : launch_static_nb<Q, 2, false>(p, P, scratch, s);
+    default: return delta ? launch_static_nb<Q, 4, true>(p, P, scratch, s) : launch_static_nb<Q, 4, false>(p, P, scratch, s);
+  }
+#endif
+}
+
+}  // namespace
+
+long long noalloc_scratch_bytes() { return (long long)EPIC_NOALLOC_SCRATCH_BYTES; }
+
+// The caller (epic_image_noalloc in epic_plan.cu) has checked: fused_ok, one layout, fused_supported.
+int fused_image_noalloc(epic_plan* p, const ImageArgs& a) {
+  float* scratch = nullptr;
+  const int sp = noalloc_scratch_ptr(&scratch);  // set-up: once per device, also on an empty call
+  if (sp != EPIC_OK) return sp;
+  if (a.n_t == 0 || a.n_chan == 0) return EPIC_OK;
+  const int Q = p->N / S;
+  FusedParams P;
+  fill_params(p, a, P);
+  const int st = Q == 2 ? launch_static_q<2>(p, P, a.n_products, scratch, a.stream)
+                        : launch_static_q<4>(p, P, a.n_products, scratch, a.stream);
+  if (st != EPIC_OK) return st;
+  p->last_launches = 2;
   return EPIC_OK;
 }
 

@@ -104,6 +104,8 @@ int fused_plan_init(epic_plan* p);  // sets p->fused_ok, allocates p->d_fused
 void fused_plan_free(epic_plan* p);
 int fused_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products);
 int fused_image(epic_plan* p, const ImageArgs& a);
+int fused_image_noalloc(epic_plan* p, const ImageArgs& a);  // the residue-group kernel with the static scratch array
+long long noalloc_scratch_bytes();
 int tensor_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products);  // tensor-core column pass
 int tensor_image(epic_plan* p, const ImageArgs& a);
 

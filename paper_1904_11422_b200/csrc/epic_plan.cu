@@ -638,6 +638,40 @@ int epic_image_host(epic_plan* plan, const void* voltages_host, int n_t, int n_c
   return EPIC_OK;
 }
 
+int epic_image_noalloc(epic_plan* plan, const void* voltages, int n_t, int n_chan, int n_pol,
+                       float* out_accum, epic_stream stream) {
+  if (!plan) return EPIC_ERR_ARG;
+  if (n_t < 0 || n_chan < 0) return EPIC_ERR_ARG;
+  if (n_pol != 1 && n_pol != 2) return EPIC_ERR_RANGE;
+  const int n_products = resolve_products(plan, n_pol);
+  const int n_planes = planes_for(n_pol, n_products);
+  if (n_planes < 0) return EPIC_ERR_RANGE;
+  plan->last_launches = 0;
+  // the residue-group kernel of epic_fused.cu: one layout, occupied cells within 32 x 32, N = 64 or 128
+  if (!plan->fused_ok || plan->n_layout != 1 || !fused_supported(plan, 0, n_pol, n_products)) return EPIC_ERR_RANGE;
+  if (plan->d_phasor && (plan->ph_n_chan != n_chan || plan->ph_n_pol != n_pol)) return EPIC_ERR_ARG;
+  if (n_t > 0 && n_chan > 0) {
+    if (!voltages || !out_accum) return EPIC_ERR_ARG;
+    if ((reinterpret_cast<uintptr_t>(voltages) & 3u) != 0) return EPIC_ERR_ARG;  // voltage rows are read as 32-bit words
+  }
+  ImageArgs a;
+  a.volt = voltages;
+  a.is_cf32 = 0;
+  a.native = plan->input_order == EPIC_ORDER_TCAP ? 1 : 0;
+  a.phasor = plan->d_phasor;
+  a.phasor_pair = plan->d_phasor_pair;
+  a.n_t = n_t;
+  a.n_chan = n_chan;
+  a.n_pol = n_pol;
+  a.n_products = n_products;
+  a.n_planes = n_planes;
+  a.out = out_accum;
+  a.stream = (cudaStream_t)stream;
+  return fused_image_noalloc(plan, a);  // looks the scratch address up (once per device), then n_t == 0 is a no-op
+}
+
+long long epic_noalloc_scratch_bytes(void) { return noalloc_scratch_bytes(); }
+
 int epic_image_cf32(epic_plan* plan, const void* voltages_cf32, int n_t, int n_chan, int n_pol,
                     float* out_accum, epic_stream stream) {
   return image_common(plan, voltages_cf32, 1, n_t, n_chan, n_pol, out_accum, stream);
@@ -743,6 +777,7 @@ const char* epic_status_string(int status) {
     case EPIC_ERR_RANGE: return "EPIC_ERR_RANGE: value outside the supported range";
     case EPIC_ERR_CUDA: return "EPIC_ERR_CUDA: a CUDA runtime call failed";
     case EPIC_ERR_NOMEM: return "EPIC_ERR_NOMEM: allocation failed";
+    case EPIC_ERR_SCRATCH: return "EPIC_ERR_SCRATCH: the call needs more than the static scratch of epic_image_noalloc (epic_noalloc_scratch_bytes()) holds";
     default: return "unknown epic_status";
   }
 }
