@@ -1003,7 +1003,8 @@ static void fill_params(const epic_plan* p, const ImageArgs& a, FusedParams& P) 
   P.n_chan = a.n_chan;
   P.n_ant = (p->n_ant + 3) & ~3;
   P.n_ant_true = p->n_ant;
-  P.unaligned = (p->n_ant & 3) != 0;
+  // rows that are not word-aligned (antenna count no multiple of 4, or a voltage pointer that is not): bytes
+  P.unaligned = (p->n_ant & 3) != 0 || (reinterpret_cast<uintptr_t>(a.volt) & 3u) != 0;
   P.n_ent = p->t.n_ent;
   P.n_pol = a.n_pol;
   P.n_planes = a.n_planes;

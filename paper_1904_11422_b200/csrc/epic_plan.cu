@@ -303,9 +303,8 @@ static int image_common(epic_plan* plan, const void* volt, int is_cf32, int n_t,
   const int tiled_can = tiled_supported(plan, is_cf32, n_pol, n_products) &&
                         (reinterpret_cast<uintptr_t>(volt) & 3u) == 0;
   int path = plan->path_req;
-  // the fused kernel reads voltage rows as 32-bit words
-  const int fused_can = fused_supported(plan, is_cf32, n_pol, n_products) &&
-                        (reinterpret_cast<uintptr_t>(volt) & 3u) == 0;
+  // (the fused kernels fetch bytes when the voltage rows are not word-aligned: any pointer will do)
+  const int fused_can = fused_supported(plan, is_cf32, n_pol, n_products);
   const int stream_can = stream_supported(plan, is_cf32, n_pol, n_products);
   // AUTO keeps the batched tiled kernels for N >= 256: measured faster than the streamed kernel;
   // the streamed kernel fetches voltages as bytes, so it takes the antenna counts the tiled row kernel cannot
@@ -652,7 +651,6 @@ int epic_image_noalloc(epic_plan* plan, const void* voltages, int n_t, int n_cha
   if (plan->d_phasor && (plan->ph_n_chan != n_chan || plan->ph_n_pol != n_pol)) return EPIC_ERR_ARG;
   if (n_t > 0 && n_chan > 0) {
     if (!voltages || !out_accum) return EPIC_ERR_ARG;
-    if ((reinterpret_cast<uintptr_t>(voltages) & 3u) != 0) return EPIC_ERR_ARG;  // voltage rows are read as 32-bit words
   }
   ImageArgs a;
   a.volt = voltages;

@@ -511,7 +511,8 @@ __device__ __forceinline__ void stream_rows_role(const StreamParams& S, float4* 
         if (e < n_e) {
           const uint32_t a = ant[e];
           if (P.native && P.n_pol == 2) {
-            pf[k] = __ldg(reinterpret_cast<const uint16_t*>(lo + 2 * a));  // (a X, a Y) adjacent bytes
+            pf[k] = __ldg(lo + 2 * a);          // (a X, a Y) adjacent bytes, fetched one by one: any pointer alignment
+            pg[k] = __ldg(lo + 2 * a + 1);
           } else {
             pf[k] = __ldg(lo + a);
             if (have_hi) pg[k] = __ldg(hi + a);

@@ -489,7 +489,7 @@ int wide_image(epic_plan* p, const ImageArgs& a) {
   P.n_chan = a.n_chan;
   P.n_ant = (p->n_ant + 3) & ~3;
   P.n_ant_true = p->n_ant;
-  P.unaligned = (p->n_ant & 3) != 0;
+  P.unaligned = (p->n_ant & 3) != 0 || (reinterpret_cast<uintptr_t>(a.volt) & 3u) != 0;  // then the prefetch reads bytes
   P.n_ent = p->t.n_ent;
   P.n_pol = a.n_pol;
   P.n_planes = a.n_planes;

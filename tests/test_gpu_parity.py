@@ -772,3 +772,40 @@ def test_image_host_matches_oracle_and_accumulates(wl, chunks):
             plan.image_host(v[:, :, :, ::2], wl.n_t, wl.n_chan, wl.n_pol, out)      # non-contiguous
         with pytest.raises(ValueError):
             plan.image_host(v, wl.n_t + 1, wl.n_chan, wl.n_pol, out)                # too short
+
+
+# ------------------------------------------------------------------ voltage pointers need no alignment
+@pytest.mark.parametrize("n_ant", [64, 77])
+def test_voltage_pointer_alignment_is_not_required(n_ant):
+    """A voltage buffer that starts 1, 2 or 3 bytes past a word boundary (a slice of a larger buffer, the second gulp of
+    an odd-sized stream): the fused, wide and streamed kernels then fetch bytes; AUTO never refuses and every path that
+    accepts the call matches the oracle.  (Found by a randomised sweep: odd antenna counts made the second of two calls
+    start at an odd byte offset, and epic_image refused a plan that epic_plan_get_path reported as fused.)"""
+    import torch
+    epic = _epic()
+    cases = [make_custom(grid_n=64, pad=2, n_ant=n_ant, n_pol=2, kernel_k=3, n_chan=3, n_t=9, layout="disc", seed=n_ant),       # fused
+             make_lwa55(n_chan=2, n_t=5, n_ant=n_ant),                                                                             # wide
+             make_custom(grid_n=128, pad=2, n_ant=n_ant, n_pol=2, kernel_k=3, n_chan=2, n_t=4, layout="uniform", seed=n_ant)]    # large grid
+    for wl in cases:
+        v = wl.voltages()
+        ref = run_oracle(wl, volt=v)
+        for native in (False, True):
+            vin = np.ascontiguousarray(np.swapaxes(v, 2, 3)) if native else v
+            refn = ref if not native else orc.epic_image(vin, wl.input_kind, wl.ant_uv, wl.taps, wl.grid_n, wl.pad, wl.n_products,
+                                                         kernel_k=wl.kernel_k, order="TCAP")
+            for shift in (1, 2, 3):
+                buf = torch.zeros(vin.size + 8, dtype=torch.uint8, device="cuda")
+                dv = buf[shift:shift + vin.size]
+                dv.copy_(torch.from_numpy(vin.reshape(-1)).cuda())
+                assert dv.data_ptr() % 4 == shift
+                with epic.Plan(wl.grid_n, wl.pad, wl.ant_uv, wl.taps, wl.kernel_k) as plan:
+                    plan.set_products(wl.n_products)
+                    if native:
+                        plan.set_input_order(epic.EPIC_ORDER_TCAP)
+                    paths = [epic.EPIC_PATH_AUTO] + ([epic.EPIC_PATH_STREAM] if wl.N == 256 else [epic.EPIC_PATH_FUSED])
+                    for path in paths:
+                        plan.set_path(path)
+                        out = torch.zeros((wl.n_chan, plan.n_planes(wl.n_pol), wl.N, wl.N), dtype=torch.float32, device="cuda")
+                        plan.image(dv, wl.n_t, wl.n_chan, wl.n_pol, out)
+                        torch.cuda.synchronize()
+                        assert_parity(out.cpu().numpy(), refn, what=f"{wl.name} shift {shift} native {native} path {path}")
