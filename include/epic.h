@@ -57,8 +57,8 @@ typedef enum epic_status {
 typedef enum epic_path {
   EPIC_PATH_AUTO = 0,
   EPIC_PATH_TWOPASS = 1, /* grid+row-FFT kernel -> scratch in global memory -> column-FFT+products kernel, batch by batch */
-  EPIC_PATH_FUSED = 2,   /* one kernel (+ a tiny ordered fix-up of split units), planes never leave the SM: N = 64, 128 with the
-                            occupied cells within 32x32 (epic_fused.cu) or within 64x64 (the wide variant, epic_wide.cu) */
+  EPIC_PATH_FUSED = 2,   /* one kernel (+ a tiny ordered fix-up of split units), planes never leave the SM: N = 32, 64, 128 with
+                            the occupied cells within 32x32 (epic_fused.cu) or, for N = 64, 128, within 64x64 (the wide variant, epic_wide.cu) */
   EPIC_PATH_TILED = 3,   /* N = 256, 512: packed row kernel -> scratch (1 GiB batches, streamed through HBM) -> packed column
                             kernel; AUTO's choice for N >= 256 */
   EPIC_PATH_TENSOR = 4,  /* the fused kernel with its column transform as a dense BF16x3 contraction on the
@@ -112,7 +112,7 @@ EPIC_API int epic_plan_destroy(epic_plan* plan);
 EPIC_API int epic_plan_set_products(epic_plan* plan, int n_products);
 
 /* Select the kernel family (testing / benchmarking): an epic_path value.  EPIC_ERR_RANGE if the plan
- * cannot use it (FUSED: occupied cells within 64x64 and N = 64 or 128; TILED, STREAM: N = 256 or 512). */
+ * cannot use it (FUSED: occupied cells within 64x64 and N = 32, 64 or 128; TILED, STREAM: N = 256 or 512). */
 EPIC_API int epic_plan_set_path(epic_plan* plan, int path);
 
 /* Tuning: bytes of the plan's scratch (the intermediate H of the tiled / two-pass paths) one batch may

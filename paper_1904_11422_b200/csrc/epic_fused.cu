@@ -788,18 +788,23 @@ template <int Q, int NPROD, bool DELTA>
 int launch_fused_nb(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
   // elements y + 16 of a row/column are read only while y < NB (the rest of the block is empty)
   const bool pc = P.cell_stride != 0, nb12 = std::max(p->R, p->Cc) <= 16 + 12;
-  if (pc)  // one layout per channel: the single-residue kernel that reloads its cell records per channel
-    return nb12 ? launch_fused<Q, NPROD, DELTA, 12, true>(p, P, s) : launch_fused<Q, NPROD, DELTA, 16, true>(p, P, s);
-  // one-layout plans: NR residues per CTA from one gather (epic_fused_dual_kernel): all four of a channel when the
-  // accumulators are 32 columns per residue (Q = 4, one or two products; C2 32.3 -> 33.5 M frames/s over two), else
-  // two.  Its shared memory is never more than the single-residue kernel's (same planes, fewer voltages), so it fits
-  // whenever fused_supported said yes.
-  constexpr int NR = (Q == 4 && NPROD != 4) ? 4 : 2;
-  if constexpr (!DELTA) {  // staged gather tables, if two CTAs still fit an SM with them
-    if (2 * (fused_dual_smem_bytes<Q>(P.n_ant, NR) + fused_stage_bytes(P.n_ent) + 1024 + 128) <= (size_t)227 * 1024)
-      return nb12 ? launch_fused_dual<Q, NPROD, false, 12, true, NR>(p, P, s) : launch_fused_dual<Q, NPROD, false, 16, true, NR>(p, P, s);
+  if constexpr (Q == 1) {  // N = 32: a single residue per axis, so no residue groups; one instantiation per layout kind
+    // two pairs per batch: the 64 threads' prefetch slots then hold up to 256 antennas
+    return pc ? launch_fused<1, NPROD, DELTA, 16, true, false, F2>(p, P, s) : launch_fused<1, NPROD, DELTA, 16, false, false, F2>(p, P, s);
+  } else {
+    if (pc)  // one layout per channel: the single-residue kernel that reloads its cell records per channel
+      return nb12 ? launch_fused<Q, NPROD, DELTA, 12, true>(p, P, s) : launch_fused<Q, NPROD, DELTA, 16, true>(p, P, s);
+    // one-layout plans: NR residues per CTA from one gather (epic_fused_dual_kernel): all four of a channel when the
+    // accumulators are 32 columns per residue (Q = 4, one or two products; C2 32.3 -> 33.5 M frames/s over two), else
+    // two.  Its shared memory is never more than the single-residue kernel's (same planes, fewer voltages), so it fits
+    // whenever fused_supported said yes.
+    constexpr int NR = (Q == 4 && NPROD != 4) ? 4 : 2;
+    if constexpr (!DELTA) {  // staged gather tables, if two CTAs still fit an SM with them
+      if (2 * (fused_dual_smem_bytes<Q>(P.n_ant, NR) + fused_stage_bytes(P.n_ent) + 1024 + 128) <= (size_t)227 * 1024)
+        return nb12 ? launch_fused_dual<Q, NPROD, false, 12, true, NR>(p, P, s) : launch_fused_dual<Q, NPROD, false, 16, true, NR>(p, P, s);
+    }
+    return nb12 ? launch_fused_dual<Q, NPROD, DELTA, 12, false, NR>(p, P, s) : launch_fused_dual<Q, NPROD, DELTA, 16, false, NR>(p, P, s);
   }
-  return nb12 ? launch_fused_dual<Q, NPROD, DELTA, 12, false, NR>(p, P, s) : launch_fused_dual<Q, NPROD, DELTA, 16, false, NR>(p, P, s);
 }
 
 template <int Q>
@@ -827,7 +832,7 @@ int fused_plan_init(epic_plan* p) {
   p->fused_ok = 0;
   p->d_fused = nullptr;
   const int Q = p->N / S;
-  if (p->N % S != 0 || (Q != 2 && Q != 4)) return EPIC_OK;
+  if (p->N % S != 0 || (Q != 1 && Q != 2 && Q != 4)) return EPIC_OK;  // N = 32 (no padding beyond the block), 64, 128
   if (p->R > S || p->Cc > S) return EPIC_OK;
   if (p->h_ent_ant.size() >= ((size_t)1 << 24)) return EPIC_OK;
   // one table of S x S cell records per layout (channel c of a per-channel plan reads table c)
@@ -952,6 +957,10 @@ int fused_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products) 
   const int Q = p->N / S;
   const int nt = 64 * Q;
   const int a_pad = (p->n_ant + 3) & ~3;  // a short tail group is fetched as bytes (prefetch_batch)
+  if (Q == 1) {  // N = 32: one residue per axis, the single-residue kernel with 64 threads
+    if ((long long)F2 * (a_pad / 4) > (long long)MAXW * nt) return 0;
+    return fused_smem_bytes<1>(a_pad, F2) <= (size_t)200 * 1024 ? 1 : 0;
+  }
   const int ff = p->n_layout > 1 ? F : F2;  // pairs per batch (at most): per-channel plans run the single-residue kernel
   if ((long long)ff * (a_pad / 4) > (long long)MAXW * nt) return 0;  // prefetch registers
   const size_t smem = p->n_layout > 1 ? (Q == 2 ? fused_smem_bytes<2>(a_pad) : fused_smem_bytes<4>(a_pad))
@@ -1012,7 +1021,7 @@ static void fill_params(const epic_plan* p, const ImageArgs& a, FusedParams& P) 
   P.Cc = p->Cc;
   // measured on C2 (R = 25): 5 pairs per batch fill the row pass's 256 lanes (250 instead of 200 tasks) but change
   // nothing (31.3 M against 31.5 M frames/s) -- the SM's other CTA already covers the idle warp; 4 stays
-  P.pairs_per_batch = F;
+  P.pairs_per_batch = p->N == S ? F2 : F;  // N = 32 runs two pairs per batch (launch_fused_nb)
   const int per_batch = a.n_pol == 2 ? P.pairs_per_batch : 2 * P.pairs_per_batch;  // time samples per batch
   P.nb = (a.n_t + per_batch - 1) / per_batch;
   P.total = (long long)a.n_chan * Q * P.nb;
@@ -1046,7 +1055,8 @@ int fused_image(epic_plan* p, const ImageArgs& a) {
   FusedParams P;
   fill_params(p, a, P);
   int st;
-  if (Q == 2) st = launch_fused_q<2>(p, P, a.n_products, a.stream);
+  if (Q == 1) st = launch_fused_q<1>(p, P, a.n_products, a.stream);
+  else if (Q == 2) st = launch_fused_q<2>(p, P, a.n_products, a.stream);
   else st = launch_fused_q<4>(p, P, a.n_products, a.stream);
   if (st != EPIC_OK) return st;
   p->last_launches = 2;  // the fused kernel and the (tiny) fix-up of split units

@@ -647,7 +647,7 @@ int epic_image_noalloc(epic_plan* plan, const void* voltages, int n_t, int n_cha
   if (n_planes < 0) return EPIC_ERR_RANGE;
   plan->last_launches = 0;
   // the residue-group kernel of epic_fused.cu: one layout, occupied cells within 32 x 32, N = 64 or 128
-  if (!plan->fused_ok || plan->n_layout != 1 || !fused_supported(plan, 0, n_pol, n_products)) return EPIC_ERR_RANGE;
+  if (!plan->fused_ok || plan->N < 64 || plan->n_layout != 1 || !fused_supported(plan, 0, n_pol, n_products)) return EPIC_ERR_RANGE;
   if (plan->d_phasor && (plan->ph_n_chan != n_chan || plan->ph_n_pol != n_pol)) return EPIC_ERR_ARG;
   if (n_t > 0 && n_chan > 0) {
     if (!voltages || !out_accum) return EPIC_ERR_ARG;

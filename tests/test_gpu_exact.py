@@ -95,6 +95,8 @@ CASES = [
     ("fused-taps-N128", 64, 2, FUSED, True),
     ("fused-delta-intgather-N64", 32, 2, FUSED, False),
     ("fused-taps-N64", 32, 2, FUSED, True),
+    ("fused-delta-intgather-N32", 16, 2, FUSED, False),
+    ("fused-taps-N32", 16, 2, FUSED, True),
     ("tensor-delta-N128", 64, 2, TENSOR, False),
     ("tensor-taps-N128", 64, 2, TENSOR, True),
     ("tiled-delta-N256", 128, 2, TILED, False),

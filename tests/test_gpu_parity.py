@@ -136,6 +136,10 @@ FUSED_CAPABLE = [
     make_custom(grid_n=32, pad=4, n_ant=100, n_pol=2, kernel_k=5, n_chan=2, n_t=7, layout="disc", n_products=4),
     make_custom(grid_n=64, pad=2, n_ant=256, n_pol=2, kernel_k=5, n_chan=2, n_t=6, layout="disc", n_products=2,
                 seed=21),                                  # 6400 gather entries: too many to stage in shared memory
+    # N = 32 (Q = 1: one residue per axis, 64-thread CTAs): C1's shape with 4+4-bit voltages, and the other product counts
+    make_custom(grid_n=16, pad=2, n_ant=16, n_pol=1, kernel_k=1, n_chan=3, n_t=21, layout="integer"),
+    make_custom(grid_n=32, pad=1, n_ant=90, n_pol=2, kernel_k=3, n_chan=2, n_t=13, layout="uniform", n_products=4),
+    make_custom(grid_n=8, pad=4, n_ant=30, n_pol=2, kernel_k=5, n_chan=40, n_t=50, layout="wrap", n_products=2),  # wraps; split units
 ]
 
 
