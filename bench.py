@@ -498,8 +498,8 @@ def run_epic(args, wl):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(volt.nbytes),
                 "d2h_bytes_per_step": int(out.numel() * 4), "measured": not args.no_e2e,
                 "how": f"one epic_image_host call (C ABI, HOST pointers: pinned voltages in, pinned out_accum out) per step: inside "
-                       f"the library {n_chunks if n_chunks else 'an automatic number of'} time chunks (the first half as long as the others), H2D of chunk k+1 on a copy "
-                       f"stream overlapped with the kernels of chunk k, one D2H of the accumulated images; synchronous call "
+                       f"the library {n_chunks if n_chunks else 'an automatic number of'} channel-range chunks (the first half as long as the others): H2D of chunk "
+                       f"k+1 and D2H of chunk k's finished images each on their own stream, overlapped with the kernels in between; synchronous call "
                        f"timed with the host clock, device idle before and after"},
         "gpu_launches": int(launches),
         "clocks": clocks,

@@ -134,13 +134,14 @@ EPIC_API int epic_image(epic_plan* plan, const void* voltages, int n_t, int n_ch
 
 /* The same gulp from HOST memory, end to end: voltages_host HOST uint8 (layout as in epic_image; pinned memory makes the
  * copies asynchronous, pageable memory works), out_accum_host HOST float[n_chan][planes][N][N].  The library cuts the gulp
- * into n_chunks time chunks (<= 0: chosen from the gulp's size, 1..8; the first one half as long, its copy is the one
- * nothing hides), copies chunk k+1
- * host->device on its own stream while epic_image of chunk k runs (double-buffered device staging owned by the plan),
- * and copies the accumulated images back.  accumulate != 0: the images are ADDED to the contents of out_accum_host (which
- * is copied to the device first); accumulate == 0: out_accum_host is overwritten.  SYNCHRONOUS: returns when
- * out_accum_host is complete.  Honours products, path, input order, delay phasors and per-channel layouts like epic_image.
- * This is the call bench.py's `e2e` leg times. */
+ * into n_chunks pieces (<= 0: chosen from the gulp's size, 1..8; the first one half as long, its copy is the one nothing
+ * hides) and pipelines them on its own streams with double-buffered device staging owned by the plan.  One-layout plans
+ * without delay phasors are cut by CHANNEL range: the host->device copy of chunk k+1 (one strided 2-D copy) and the
+ * device->host copy of chunk k's finished images both overlap the kernels in between.  Other plans are cut in TIME: the
+ * host->device copies overlap the kernels and the accumulated images are copied back once at the end.
+ * accumulate != 0: the images are ADDED to the contents of out_accum_host (which is copied to the device first);
+ * accumulate == 0: out_accum_host is overwritten.  SYNCHRONOUS: returns when out_accum_host is complete.  Honours products,
+ * path, input order, delay phasors and per-channel layouts like epic_image.  This is the call bench.py's `e2e` leg times. */
 EPIC_API int epic_image_host(epic_plan* plan, const void* voltages_host, int n_t, int n_chan, int n_pol,
                     float* out_accum_host, int accumulate, int n_chunks);
 

@@ -36,7 +36,7 @@ struct DevTables {
 namespace epic {
 // epic_image_host: double-buffered device staging of the voltages, a device copy of out_accum, two streams
 struct HostPipe {
-  cudaStream_t compute, copy;
+  cudaStream_t compute, copy, back;  // kernels; host->device copies; device->host copies of finished channel chunks
   cudaEvent_t copied[2], consumed[2];
   void* d_volt[2];
   size_t volt_bytes;   // capacity of each staging buffer

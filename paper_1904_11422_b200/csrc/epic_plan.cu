@@ -342,6 +342,7 @@ static void host_pipe_free(epic_plan* plan) {
   if (hp->d_out) cudaFree(hp->d_out);
   if (hp->compute) cudaStreamDestroy(hp->compute);
   if (hp->copy) cudaStreamDestroy(hp->copy);
+  if (hp->back) cudaStreamDestroy(hp->back);
   delete hp;
   plan->pipe = nullptr;
 }
@@ -355,6 +356,7 @@ static int host_pipe_prepare(epic_plan* plan, size_t chunk_bytes, size_t out_byt
     plan->pipe = hp;
     EPIC_CUDA_TRY(cudaStreamCreateWithFlags(&hp->compute, cudaStreamNonBlocking));
     EPIC_CUDA_TRY(cudaStreamCreateWithFlags(&hp->copy, cudaStreamNonBlocking));
+    EPIC_CUDA_TRY(cudaStreamCreateWithFlags(&hp->back, cudaStreamNonBlocking));
     for (int i = 0; i < 2; ++i) {
       EPIC_CUDA_TRY(cudaEventCreateWithFlags(&hp->copied[i], cudaEventDisableTiming));
       EPIC_CUDA_TRY(cudaEventCreateWithFlags(&hp->consumed[i], cudaEventDisableTiming));
@@ -594,43 +596,80 @@ int epic_image_host(epic_plan* plan, const void* voltages_host, int n_t, int n_c
   if (!out_accum_host || (n_t > 0 && !voltages_host)) return EPIC_ERR_ARG;
   const size_t sample_bytes = (size_t)n_chan * n_pol * plan->n_ant;  // one time sample of all channels
   const size_t out_bytes = (size_t)n_chan * n_planes * plan->N * plan->N * sizeof(float);
-  // automatic chunk count: the first chunk's copy is exposed (~ bytes / (2 n) at ~50 GB/s) and every chunk costs a
-  // call (~0.1 ms of launches, flush and fix-up), so n ~ sqrt(bytes / 8 MB): C2 (65.5 MB) 2, C3 (164 MB) 4 (measured on C2: 2 chunks 27.7, 3 27.2, 4 26.8, 6 25.4 M frames/s)
-  if (n_chunks <= 0) n_chunks = std::max(1, std::min(8, (int)std::sqrt((double)n_t * (double)sample_bytes / 8.0e6)));
-  n_chunks = std::max(1, std::min(n_chunks, n_t));
+  // Two ways to cut the gulp.  By CHANNEL range (one-layout plans without delay phasors, enough channels): a chunk's
+  // images are final when its kernels end, so the device->host copy of chunk k overlaps the kernels of chunk k+1 just
+  // as the host->device copy of chunk k+1 overlaps those of chunk k; the chunk's voltages are a strided slice of the
+  // host array ([T][C][Np][A]: one 2-D copy).  By TIME otherwise: the images are read back once, at the end.
+  // Automatic chunk count: the first chunk's copy is exposed and every chunk costs a call (launches, fix-up), so
+  // n ~ sqrt(bytes / 8 MB), 1..8; sqrt(bytes / 4 MB) for the channel cut, whose read-back overlaps too.
+  const bool chan_ok = plan->n_layout == 1 && !plan->d_phasor && n_t > 0;
+  if (n_chunks <= 0) {  // measured on C2 (65.5 MB), channel cut: 2 chunks 30.0, 3 31.1, 4 31.5, 6 31.1, 8 30.1 M frames/s
+    const double bytes = (double)n_t * (double)sample_bytes;
+    n_chunks = std::max(1, std::min(8, (int)std::sqrt(bytes / (chan_ok ? 4.0e6 : 8.0e6))));
+  }
+  const bool by_channel = chan_ok && n_chan >= 2 * n_chunks && n_chunks > 1;
+  const int extent = by_channel ? n_chan : n_t;
+  n_chunks = std::max(1, std::min(n_chunks, extent));
   // chunk edges: a short first chunk (its copy is the one nothing can hide), the rest equal
   std::vector<int> edge(1, 0);
-  const int first = (n_chunks > 1 && n_t >= 4 * n_chunks) ? n_t / (2 * n_chunks) : 0;
+  const int first = (n_chunks > 1 && extent >= 4 * n_chunks) ? extent / (2 * n_chunks) : 0;
   if (first) edge.push_back(first);
   const int rest = n_chunks - (first ? 1 : 0);
-  for (int k = 1; k <= rest; ++k) edge.push_back(first + (int)((long long)(n_t - first) * k / rest));
+  for (int k = 1; k <= rest; ++k) edge.push_back(first + (int)((long long)(extent - first) * k / rest));
   int chunk_max = 0;
   for (size_t k = 0; k + 1 < edge.size(); ++k) chunk_max = std::max(chunk_max, edge[k + 1] - edge[k]);
-  int st = host_pipe_prepare(plan, std::max<size_t>(16, (size_t)chunk_max * sample_bytes), out_bytes);
+  const size_t chan_bytes = (size_t)n_pol * plan->n_ant;                       // one channel of one time sample
+  const size_t img_floats = (size_t)n_planes * plan->N * plan->N;              // one channel's images
+  const size_t chunk_bytes = by_channel ? (size_t)chunk_max * chan_bytes * n_t : (size_t)chunk_max * sample_bytes;
+  int st = host_pipe_prepare(plan, std::max<size_t>(16, chunk_bytes), out_bytes);
   if (st != EPIC_OK) return st;
   HostPipe* hp = plan->pipe;
-  if (accumulate) EPIC_CUDA_TRY(cudaMemcpyAsync(hp->d_out, out_accum_host, out_bytes, cudaMemcpyHostToDevice, hp->compute));
-  else EPIC_CUDA_TRY(cudaMemsetAsync(hp->d_out, 0, out_bytes, hp->compute));
   int launches = 0;
   const uint8_t* src = static_cast<const uint8_t*>(voltages_host);
-  for (size_t k = 0; k + 1 < edge.size(); ++k) {
-    const int a = edge[k], b = edge[k + 1], buf = (int)(k & 1);
-    if (b == a) continue;
-    if (k >= 2) EPIC_CUDA_TRY(cudaStreamWaitEvent(hp->copy, hp->consumed[buf], 0));  // the kernels that read this buffer are done
-    EPIC_CUDA_TRY(cudaMemcpyAsync(hp->d_volt[buf], src + (size_t)a * sample_bytes, (size_t)(b - a) * sample_bytes,
-                                  cudaMemcpyHostToDevice, hp->copy));
-    EPIC_CUDA_TRY(cudaEventRecord(hp->copied[buf], hp->copy));
-    EPIC_CUDA_TRY(cudaStreamWaitEvent(hp->compute, hp->copied[buf], 0));
-    st = image_common(plan, hp->d_volt[buf], 0, b - a, n_chan, n_pol, hp->d_out, hp->compute);
-    if (st != EPIC_OK) break;
-    launches += plan->last_launches;
-    EPIC_CUDA_TRY(cudaEventRecord(hp->consumed[buf], hp->compute));
+  if (by_channel) {
+    for (size_t k = 0; k + 1 < edge.size(); ++k) {
+      const int c0 = edge[k], c1 = edge[k + 1], buf = (int)(k & 1);
+      if (c1 == c0) continue;
+      const size_t width = (size_t)(c1 - c0) * chan_bytes;
+      float* d_img = hp->d_out + (size_t)c0 * img_floats;
+      const size_t img_bytes = (size_t)(c1 - c0) * img_floats * sizeof(float);
+      if (k >= 2) EPIC_CUDA_TRY(cudaStreamWaitEvent(hp->copy, hp->consumed[buf], 0));  // the kernels that read this buffer are done
+      EPIC_CUDA_TRY(cudaMemcpy2DAsync(hp->d_volt[buf], width, src + (size_t)c0 * chan_bytes, sample_bytes, width, (size_t)n_t,
+                                      cudaMemcpyHostToDevice, hp->copy));
+      if (accumulate)
+        EPIC_CUDA_TRY(cudaMemcpyAsync(d_img, out_accum_host + (size_t)c0 * img_floats, img_bytes, cudaMemcpyHostToDevice, hp->copy));
+      EPIC_CUDA_TRY(cudaEventRecord(hp->copied[buf], hp->copy));
+      if (!accumulate) EPIC_CUDA_TRY(cudaMemsetAsync(d_img, 0, img_bytes, hp->compute));
+      EPIC_CUDA_TRY(cudaStreamWaitEvent(hp->compute, hp->copied[buf], 0));
+      st = image_common(plan, hp->d_volt[buf], 0, n_t, c1 - c0, n_pol, d_img, hp->compute);
+      if (st != EPIC_OK) break;
+      launches += plan->last_launches;
+      EPIC_CUDA_TRY(cudaEventRecord(hp->consumed[buf], hp->compute));
+      EPIC_CUDA_TRY(cudaStreamWaitEvent(hp->back, hp->consumed[buf], 0));  // (waits for the record just made, not for later ones)
+      EPIC_CUDA_TRY(cudaMemcpyAsync(out_accum_host + (size_t)c0 * img_floats, d_img, img_bytes, cudaMemcpyDeviceToHost, hp->back));
+    }
+  } else {
+    if (accumulate) EPIC_CUDA_TRY(cudaMemcpyAsync(hp->d_out, out_accum_host, out_bytes, cudaMemcpyHostToDevice, hp->compute));
+    else EPIC_CUDA_TRY(cudaMemsetAsync(hp->d_out, 0, out_bytes, hp->compute));
+    for (size_t k = 0; k + 1 < edge.size(); ++k) {
+      const int a = edge[k], b = edge[k + 1], buf = (int)(k & 1);
+      if (b == a) continue;
+      if (k >= 2) EPIC_CUDA_TRY(cudaStreamWaitEvent(hp->copy, hp->consumed[buf], 0));  // the kernels that read this buffer are done
+      EPIC_CUDA_TRY(cudaMemcpyAsync(hp->d_volt[buf], src + (size_t)a * sample_bytes, (size_t)(b - a) * sample_bytes,
+                                    cudaMemcpyHostToDevice, hp->copy));
+      EPIC_CUDA_TRY(cudaEventRecord(hp->copied[buf], hp->copy));
+      EPIC_CUDA_TRY(cudaStreamWaitEvent(hp->compute, hp->copied[buf], 0));
+      st = image_common(plan, hp->d_volt[buf], 0, b - a, n_chan, n_pol, hp->d_out, hp->compute);
+      if (st != EPIC_OK) break;
+      launches += plan->last_launches;
+      EPIC_CUDA_TRY(cudaEventRecord(hp->consumed[buf], hp->compute));
+    }
+    if (st == EPIC_OK) EPIC_CUDA_TRY(cudaMemcpyAsync(out_accum_host, hp->d_out, out_bytes, cudaMemcpyDeviceToHost, hp->compute));
   }
-  if (st == EPIC_OK) EPIC_CUDA_TRY(cudaMemcpyAsync(out_accum_host, hp->d_out, out_bytes, cudaMemcpyDeviceToHost, hp->compute));
-  const cudaError_t c1 = cudaStreamSynchronize(hp->copy), c2 = cudaStreamSynchronize(hp->compute);
+  const cudaError_t c1e = cudaStreamSynchronize(hp->copy), c2e = cudaStreamSynchronize(hp->compute), c3e = cudaStreamSynchronize(hp->back);
   if (st != EPIC_OK) return st;
-  if (c1 != cudaSuccess || c2 != cudaSuccess) {
-    set_cuda_error(c1 != cudaSuccess ? c1 : c2);
+  if (c1e != cudaSuccess || c2e != cudaSuccess || c3e != cudaSuccess) {
+    set_cuda_error(c1e != cudaSuccess ? c1e : (c2e != cudaSuccess ? c2e : c3e));
     return EPIC_ERR_CUDA;
   }
   plan->last_launches = launches;
