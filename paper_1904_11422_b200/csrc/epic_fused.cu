@@ -316,9 +316,11 @@ __global__ void __launch_bounds__(64 * Q) epic_fused_dual_fixup(FusedParams P, i
 
 // NRES residues per CTA: 2, or all 4 (Q = 4, one or two products: 4 x 32 accumulator columns per thread) with one
 // pair per batch; the work per batch is the same 4 (pair, residue) column tasks per thread either way.
-template <int Q, int NPROD, bool DELTA, int NB, bool STG, int NRES>
+// PC: every channel has its own cell table (per-channel plans, reading Q15): the thread's cell records are
+// reloaded when the work list crosses into the next channel (a separate instantiation, as for the single-residue kernel).
+template <int Q, int NPROD, bool DELTA, int NB, bool STG, int NRES, bool PC = false>
 __global__ void __launch_bounds__(64 * Q, 2) epic_fused_dual_kernel(FusedParams P) {
-  static_assert(!(STG && DELTA), "staged tables: tap kernels only");
+  static_assert(!(STG && (DELTA || PC)), "staged tables: tap kernels of one-layout plans only");
   static_assert(NRES == 2 || (NRES == 4 && Q == 4 && NPROD != 4), "four residues: Q = 4, accumulators of 32 columns");
   constexpr int NT = 64 * Q, N = 32 * Q, HQ = Q / NRES, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1);
   constexpr int FB = 4 / NRES;               // pairs per batch
@@ -341,7 +343,8 @@ __global__ void __launch_bounds__(64 * Q, 2) epic_fused_dual_kernel(FusedParams 
   int unit = (int)(g0 / P.nb);  // unit = (channel, group of NRES residues)
   uint2 info[S * S / NT];
 #pragma unroll
-  for (int j = 0; j < S * S / NT; ++j) info[j] = __ldg(P.cell_info + tid + j * NT);
+  for (int j = 0; j < S * S / NT; ++j)
+    info[j] = __ldg(P.cell_info + (PC ? (size_t)(unit / HQ) * (S * S) : (size_t)0) + tid + j * NT);
   for (int i = tid; i < NRES * SET; i += NT) gA[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);  // rows >= R stay zero
   for (int i = tid; i < 2 * Q * TWV; i += NT) tws[i] = __ldg(P.tw + i);
   float2* tap_s = reinterpret_cast<float2*>(E + FB * P.n_ant);
@@ -453,6 +456,13 @@ __global__ void __launch_bounds__(64 * Q, 2) epic_fused_dual_kernel(FusedParams 
     if (unit_n != unit || !more) {
       flush(unit, seg_begin == 0 && b == P.nb - 1, unit == first_unit ? 0 : 1);
       seg_begin = 0;
+    }
+    if constexpr (PC) {
+      if (unit_n / HQ != unit / HQ && more) {  // the next channel's cells (this batch's gather is done with these)
+#pragma unroll
+        for (int j = 0; j < S * S / NT; ++j)
+          info[j] = __ldg(P.cell_info + (size_t)(unit_n / HQ) * (S * S) + tid + j * NT);
+      }
     }
     unit = unit_n; b = b_n;
     __syncthreads();  // next batch's E is complete; the planes are free
@@ -763,7 +773,7 @@ int launch_fused(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
 }
 
 // dual-residue kernel (one layout): sized for two CTAs per SM
-template <int Q, int NPROD, bool DELTA, int NB, bool STG, int NRES = 2>
+template <int Q, int NPROD, bool DELTA, int NB, bool STG, int NRES = 2, bool PC = false>
 int launch_fused_dual(const epic_plan* p, FusedParams P, cudaStream_t s) {
   constexpr int NT = 64 * Q, NACC = NPROD == 4 ? 4 : (NPROD == 2 ? 2 : 1), FB = 4 / NRES;
   P.pairs_per_batch = FB;
@@ -771,7 +781,7 @@ int launch_fused_dual(const epic_plan* p, FusedParams P, cudaStream_t s) {
   P.nb = (P.n_t + per_batch - 1) / per_batch;
   P.total = (long long)P.n_chan * (Q / NRES) * P.nb;
   const size_t smem = fused_dual_smem_bytes<Q>(P.n_ant, NRES) + (STG ? fused_stage_bytes(P.n_ent) : 0);
-  auto kern = epic_fused_dual_kernel<Q, NPROD, DELTA, NB, STG, NRES>;
+  auto kern = epic_fused_dual_kernel<Q, NPROD, DELTA, NB, STG, NRES, PC>;
   if (smem > 48 * 1024)
     EPIC_CUDA_TRY(cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   // tensor-memory kernels: the occupancy query answers 1; two CTAs (at most 2 x 256 of the 512 columns) share an SM
@@ -792,13 +802,14 @@ int launch_fused_nb(const epic_plan* p, const FusedParams& P, cudaStream_t s) {
     // two pairs per batch: the 64 threads' prefetch slots then hold up to 256 antennas
     return pc ? launch_fused<1, NPROD, DELTA, 16, true, false, F2>(p, P, s) : launch_fused<1, NPROD, DELTA, 16, false, false, F2>(p, P, s);
   } else {
-    if (pc)  // one layout per channel: the single-residue kernel that reloads its cell records per channel
-      return nb12 ? launch_fused<Q, NPROD, DELTA, 12, true>(p, P, s) : launch_fused<Q, NPROD, DELTA, 16, true>(p, P, s);
-    // one-layout plans: NR residues per CTA from one gather (epic_fused_dual_kernel): all four of a channel when the
+    // NR residues per CTA from one gather (epic_fused_dual_kernel): all four of a channel when the
     // accumulators are 32 columns per residue (Q = 4, one or two products; C2 32.3 -> 33.5 M frames/s over two), else
     // two.  Its shared memory is never more than the single-residue kernel's (same planes, fewer voltages), so it fits
     // whenever fused_supported said yes.
     constexpr int NR = (Q == 4 && NPROD != 4) ? 4 : 2;
+    if (pc)  // one layout per channel: the instantiation that reloads its cell records when the channel changes
+      return nb12 ? launch_fused_dual<Q, NPROD, DELTA, 12, false, NR, true>(p, P, s)
+                  : launch_fused_dual<Q, NPROD, DELTA, 16, false, NR, true>(p, P, s);
     if constexpr (!DELTA) {  // staged gather tables, if two CTAs still fit an SM with them
       if (2 * (fused_dual_smem_bytes<Q>(P.n_ant, NR) + fused_stage_bytes(P.n_ent) + 1024 + 128) <= (size_t)227 * 1024)
         return nb12 ? launch_fused_dual<Q, NPROD, false, 12, true, NR>(p, P, s) : launch_fused_dual<Q, NPROD, false, 16, true, NR>(p, P, s);
@@ -961,10 +972,8 @@ int fused_supported(const epic_plan* p, int is_cf32, int n_pol, int n_products) 
     if ((long long)F2 * (a_pad / 4) > (long long)MAXW * nt) return 0;
     return fused_smem_bytes<1>(a_pad, F2) <= (size_t)200 * 1024 ? 1 : 0;
   }
-  const int ff = p->n_layout > 1 ? F : F2;  // pairs per batch (at most): per-channel plans run the single-residue kernel
-  if ((long long)ff * (a_pad / 4) > (long long)MAXW * nt) return 0;  // prefetch registers
-  const size_t smem = p->n_layout > 1 ? (Q == 2 ? fused_smem_bytes<2>(a_pad) : fused_smem_bytes<4>(a_pad))
-                                      : (Q == 2 ? fused_dual_smem_bytes<2>(a_pad) : fused_dual_smem_bytes<4>(a_pad));
+  if ((long long)F2 * (a_pad / 4) > (long long)MAXW * nt) return 0;  // prefetch registers (at most F2 pairs per batch)
+  const size_t smem = Q == 2 ? fused_dual_smem_bytes<2>(a_pad) : fused_dual_smem_bytes<4>(a_pad);
   return smem <= (size_t)200 * 1024 ? 1 : 0;
 }
 
