@@ -172,14 +172,39 @@ def input_fingerprint(wl, volt) -> dict:
 def measured_traffic(wl_name: str, path: int):
     """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of this workload and kernel family
     from the ncu captures summarised in profiles/traffic.csv, or None."""
+    row = _profile_row(wl_name, path)
+    try:
+        return int(row[1]) if row and row[1] else None
+    except ValueError:
+        return None
+
+
+def _profile_row(wl_name: str, path: int):
+    """Row of profiles/traffic.csv for this workload and kernel family: [key, dram bytes per launch, FMA-pipe busy %,
+    issue slots busy %] from the ncu --set full capture named in profiles/traffic.md, or None."""
     tpath = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
         with open(tpath) as fh:
-            rows = dict(ln.strip().split(",")[:2] for ln in fh.read().splitlines()[1:] if "," in ln)
-        key = f"{wl_name}:{PATH_NAMES.get(path)}"
-        return int(rows[key]) if key in rows else None
-    except (OSError, ValueError):
-        return None
+            for ln in fh.read().splitlines()[1:]:
+                f = [x.strip() for x in ln.split(",")]
+                if f and f[0] == f"{wl_name}:{PATH_NAMES.get(path)}":
+                    return f + [""] * (4 - len(f))
+    except OSError:
+        pass
+    return None
+
+
+def measured_pipe_busy(wl_name: str, path: int) -> dict:
+    """What the dominant kernel EXECUTES, beside the algorithmic fraction: sm__pipe_fma_cycles_active and
+    smsp__issue_active (% of peak) of the same ncu capture as `traffic`; None where no capture has them."""
+    row = _profile_row(wl_name, path)
+    def num(x):
+        try:
+            return float(x)
+        except (TypeError, ValueError):
+            return None
+    return {"fma_pipe_busy_pct": num(row[2]) if row else None, "issue_slots_busy_pct": num(row[3]) if row else None,
+            "source": "profiles/traffic.csv (ncu --set full capture, see profiles/traffic.md)"}
 
 
 def roofline_of(wl, kernel_ms: float, path: int, probe_tflops=None) -> dict:
@@ -201,6 +226,7 @@ def roofline_of(wl, kernel_ms: float, path: int, probe_tflops=None) -> dict:
         "algorithmic_bytes_per_launch": bytes_f * wl.frames,
         "hbm_achieved_gbs": bytes_f * wl.frames / (kernel_ms * 1e-3) / 1e9,
         "kernel_ms": kernel_ms, "kernel": PATH_KERNELS.get(path, str(path)),
+        "executed": measured_pipe_busy(wl.name, path),
     }
     if probe_tflops:
         r["peak_measured_fma_probe"] = probe_tflops
