@@ -115,3 +115,35 @@ def test_binding_rejects_host_tensors_for_device_pointers():
         binding._check_tensor(torch.zeros(16, dtype=torch.uint8), "voltages", "uint8", 16, None)
     binding._check_tensor(1234, "voltages", "uint8", 16, None)   # raw addresses are the caller's business, as in C
     binding._check_tensor(None, "voltages", "uint8", 16, None)
+
+
+def test_header_is_plain_c_and_a_c_program_links_and_fails_loudly_without_a_gpu(tmp_path):
+    """include/epic.h is a C ABI: it compiles as C99 with gcc, a C program links against libepic.so with no C++ or
+    torch in sight, and without a CUDA device the library reports EPIC_ERR_CUDA (there is no CPU fallback); with a
+    device the same program succeeds."""
+    import shutil
+    import subprocess
+    from paper_1904_11422_b200 import binding
+    from paper_1904_11422_b200.build import build
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        import pytest
+        pytest.skip("no gcc")
+    build()
+    inc = os.path.join(ROOT, "include")
+    subprocess.run([gcc, "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-fsyntax-only", "-x", "c",
+                    os.path.join(inc, "epic.h")], check=True)
+    src = tmp_path / "use_epic.c"
+    src.write_text('#include "epic.h"\n#include <stdio.h>\n'
+                   'int main(void) {\n  epic_plan* p = 0;\n  float uv[2] = {1.0f, 2.0f};\n'
+                   '  int st = epic_plan_create(&p, 16, 2, 1, uv, 0, 1);\n'
+                   '  printf("%d|%s|%lld\\n", st, epic_status_string(st), epic_noalloc_scratch_bytes());\n'
+                   '  epic_plan_destroy(p);\n  return 0;\n}\n')
+    exe = tmp_path / "use_epic"
+    libdir = os.path.dirname(binding.LIB_PATH)
+    subprocess.run([gcc, "-std=c99", "-Wall", "-I", inc, str(src), "-o", str(exe), "-L", libdir, "-l:libepic.so",
+                    f"-Wl,-rpath,{libdir}"], check=True)
+    out = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.strip().split("|")
+    assert int(out[0]) in (binding.EPIC_OK, binding.EPIC_ERR_CUDA), out
+    assert out[1].startswith("EPIC_OK") or out[1].startswith("EPIC_ERR_CUDA"), out
+    assert int(out[2]) == 80 << 20
