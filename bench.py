@@ -9,6 +9,13 @@ N=1 times configs[1] (C2, the LWA-station-like case BASELINE.json's target is qu
 For N>1 (torchrun, one rank per GPU) every rank images its own copy of the workload -- channels
 are independent, so the path shards with no collective ("weak" scaling).
 Rank 0 prints ONE JSON line.  `--impl reference` times the float64 CPU oracle instead.
+
+The line carries: `value` (device-resident inputs, CUDA events), `e2e` (one epic_image_host call per step: pinned host
+voltages in, host images out, copies inside the timed region), `roofline` (algorithmic flops and bytes against the FP32
+and HBM peaks, `bound` = the slower side, measured DRAM `traffic` and pipe-busy `executed` from the ncu captures under
+profiles/), `clocks`, `cpu_baseline` (the oracle on one core and on all cores), and -- default C2 run only --
+`other_configs` (C3, C4, C5, the streamed and tensor-core variants, the wide-support workloads).
+`--sweep grid|gulp` prints the paper-figure analogues (Fig. 7, 8), one JSON line per point.
 """
 from __future__ import annotations
 

@@ -67,7 +67,8 @@ typedef enum epic_path {
   EPIC_PATH_STREAM = 5   /* N = 256, 512: ONE persistent kernel; row CTAs hand row-transformed frames to column CTAs
                             through a ring that stays in L2, accumulators live in registers for the whole call:
                             HBM sees the voltages and out_accum once.  Measured slower than
-                            EPIC_PATH_TILED so far, so AUTO does not pick it; EPIC_ERR_RANGE at epic_image time if one
+                            EPIC_PATH_TILED so far, so AUTO picks it only where the tiled row kernel cannot run (antenna counts that
+                            are no multiple of 4, voltage pointers that are not word-aligned); EPIC_ERR_RANGE at epic_image time if one
                             channel's row and column CTAs cannot be co-resident */
 } epic_path;
 
@@ -115,7 +116,7 @@ EPIC_API int epic_plan_set_products(epic_plan* plan, int n_products);
  * cannot use it (FUSED: occupied cells within 64x64 and N = 32, 64 or 128; TILED, STREAM: N = 256 or 512). */
 EPIC_API int epic_plan_set_path(epic_plan* plan, int path);
 
-/* Tuning: bytes of the plan's scratch (the intermediate H of the tiled / two-pass paths) one batch may
+/* Tuning: bytes of the plan's scratch (the intermediate H of the tiled / two-pass paths; the ring of the streamed path) one batch may
  * use; 0 = all of it (1 GiB for N >= 256, else 128 MiB).  A small limit (e.g. 64 MiB) keeps H resident in
  * the 126 MB L2 at the price of more, shorter batches, each ending in one read-modify-write of its
  * channels' out_accum.  A batch always holds at least one frame. */
